@@ -1,0 +1,166 @@
+"""ctypes wrapper of the CPU oracle (oracle/oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It never imports the CUDA package's library or binding.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle.so")
+_SRC = os.path.join(_HERE, "oracle.c")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle.c with gcc (+OpenMP)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-o", _SO, _SRC, "-lm"]
+        )
+    return _SO
+
+
+class Options(C.Structure):
+    _fields_ = [("tau", C.c_double), ("density_weighted", C.c_int32), ("sample_mod", C.c_uint32), ("sample_seed", C.c_uint32)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets")]
+
+    def asdict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_SO)
+    return _lib
+
+
+def _sys_args(sysm):
+    xyz = np.ascontiguousarray(sysm.xyz, dtype=np.float64)
+    sh = np.ascontiguousarray(sysm.shells, dtype=np.int32)
+    ex = np.ascontiguousarray(sysm.exps, dtype=np.float64)
+    co = np.ascontiguousarray(sysm.coefs, dtype=np.float64)
+    keep = (xyz, sh, ex, co)
+    args = (
+        C.c_int(xyz.shape[0]), xyz.ctypes.data_as(C.c_void_p), C.c_int(sh.shape[0]), sh.ctypes.data_as(C.c_void_p),
+        C.c_int(ex.shape[0]), ex.ctypes.data_as(C.c_void_p), co.ctypes.data_as(C.c_void_p),
+    )
+    return args, keep
+
+
+def _ncart(l):
+    return (l + 1) * (l + 2) // 2
+
+
+def boys(mmax: int, T: float) -> np.ndarray:
+    out = np.zeros(mmax + 1)
+    lib().orc_boys(C.c_int(mmax), C.c_double(T), out.ctypes.data_as(C.c_void_p))
+    return out
+
+
+def boys_op(mmax: int, T: float, rho: float, omega: float) -> np.ndarray:
+    out = np.zeros(mmax + 1)
+    lib().orc_boys_op(C.c_int(mmax), C.c_double(T), C.c_double(rho), C.c_double(omega), out.ctypes.data_as(C.c_void_p))
+    return out
+
+
+def eri_shell(sysm, i, j, k, l, omega=0.0, deriv=False):
+    args, keep = _sys_args(sysm)
+    ls = [int(sysm.shells[s, 1]) for s in (i, j, k, l)]
+    shape = tuple(_ncart(x) for x in ls)
+    out = np.zeros(shape)
+    dout = np.zeros((4, 3) + shape) if deriv else None
+    rc = lib().orc_eri_shell(*args, C.c_int(i), C.c_int(j), C.c_int(k), C.c_int(l), C.c_double(omega),
+                             out.ctypes.data_as(C.c_void_p), dout.ctypes.data_as(C.c_void_p) if deriv else None)
+    assert rc == 0, rc
+    return (out, dout) if deriv else out
+
+
+def eri_tensor(sysm, omega=0.0):
+    args, keep = _sys_args(sysm)
+    n = sysm.nbf
+    out = np.zeros((n, n, n, n))
+    rc = lib().orc_eri_tensor(*args, C.c_double(omega), out.ctypes.data_as(C.c_void_p))
+    assert rc == 0, rc
+    return out
+
+
+def overlap(sysm):
+    args, keep = _sys_args(sysm)
+    n = sysm.nbf
+    out = np.zeros((n, n))
+    rc = lib().orc_overlap(*args, out.ctypes.data_as(C.c_void_p))
+    assert rc == 0, rc
+    return out
+
+
+def schwarz(sysm):
+    args, keep = _sys_args(sysm)
+    n = sysm.nshell
+    out = np.zeros((n, n))
+    rc = lib().orc_schwarz(*args, out.ctypes.data_as(C.c_void_p))
+    assert rc == 0, rc
+    return out
+
+
+def _mats(pairs):
+    A = [np.ascontiguousarray(a, dtype=np.float64) for a, _ in pairs]
+    B = [np.ascontiguousarray(b, dtype=np.float64) for _, b in pairs]
+    PA = (C.c_void_p * len(A))(*[a.ctypes.data for a in A])
+    PB = (C.c_void_p * len(B))(*[b.ctypes.data for b in B])
+    return PA, PB, (A, B)
+
+
+def _call(fn, sysm, pairs, wJ, wK, cJ, cK, cLR, omega, nout, tau=None, density_weighted=None, sample_mod=0, sample_seed=0):
+    args, keep = _sys_args(sysm)
+    PA, PB, keep2 = _mats(pairs)
+    wJ = np.ascontiguousarray(wJ, dtype=np.float64)
+    wK = np.ascontiguousarray(wK, dtype=np.float64)
+    opt = Options(sysm.tau if tau is None else tau,
+                  sysm.density_weighted if density_weighted is None else density_weighted, sample_mod, sample_seed)
+    st = Stats()
+    out = np.zeros(nout)
+    rc = fn(*args, C.byref(opt), C.c_int(len(pairs)), PA, PB, wJ.ctypes.data_as(C.c_void_p), wK.ctypes.data_as(C.c_void_p),
+            C.c_double(cJ), C.c_double(cK), C.c_double(cLR), C.c_double(omega), out.ctypes.data_as(C.c_void_p), C.byref(st))
+    assert rc == 0, rc
+    return out, st.asdict()
+
+
+def gradient(sysm, pairs, wJ, wK, cJ, cK, cLR, omega, **kw):
+    g, st = _call(lib().orc_gradient, sysm, pairs, wJ, wK, cJ, cK, cLR, omega, 3 * sysm.natom, **kw)
+    return g.reshape(-1, 3), st
+
+
+def energy(sysm, pairs, wJ, wK, cJ, cK, cLR, omega, **kw):
+    e, st = _call(lib().orc_energy, sysm, pairs, wJ, wK, cJ, cK, cLR, omega, 1, **kw)
+    return float(e[0]), st
+
+
+def gradient_n4(sysm, pairs, wJ, wK, cJ, cK, cLR, omega):
+    args, keep = _sys_args(sysm)
+    PA, PB, keep2 = _mats(pairs)
+    wJ = np.ascontiguousarray(wJ, dtype=np.float64)
+    wK = np.ascontiguousarray(wK, dtype=np.float64)
+    out = np.zeros(3 * sysm.natom)
+    rc = lib().orc_gradient_n4(*args, C.c_int(len(pairs)), PA, PB, wJ.ctypes.data_as(C.c_void_p), wK.ctypes.data_as(C.c_void_p),
+                               C.c_double(cJ), C.c_double(cK), C.c_double(cLR), C.c_double(omega), out.ctypes.data_as(C.c_void_p))
+    assert rc == 0, rc
+    return out.reshape(-1, 3)
+
+
+def sample_keep(i, j, k, l, mod, seed) -> bool:
+    return bool(lib().orc_sample_keep(C.c_int(i), C.c_int(j), C.c_int(k), C.c_int(l), C.c_uint32(mod), C.c_uint32(seed)))
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
