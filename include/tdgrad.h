@@ -1,0 +1,123 @@
+/*
+ * tdgrad.h — C ABI of libtdgrad.so: integral-direct ERI-derivative gradient on one B200 (sm_100a).
+ *
+ * What the library computes (PAPER.md = /root/reference/PAPER.md, arXiv 2407.16586):
+ *
+ *   E(R)    = sum_k [ wJ_k cJ J(A_k,B_k) - wK_k ( cK K(A_k,B_k) + cLR K_w(A_k,B_k) ) ]
+ *   J(A,B)  = sum A_mn B_ls (mn|ls)      K(A,B) = sum A_ml B_ns (mn|ls)      K_w: (mn|ls)_lr
+ *   grad[E][x] = dE/dR_{E,x}   with all matrices held fixed
+ *
+ * i.e. the 4th and 5th terms of eq 7 with the density products of eqs 13-14
+ * (PAPER.md:110-114); (mn|ls) uses 1/r (eqs 3-4), (mn|ls)_lr uses erf(omega r)/r
+ * (eq 5); basis functions are contracted Cartesian Gaussians (eqs 38, 43, PAPER.md:234-241,
+ * 268-273); centre derivatives by eq 39/42; one centre by translational
+ * invariance (eq 41); algorithm of Fig. 1; pair list sorted by
+ * contraction degree and Schwarz bound, one kernel per angular class; Rys quadrature
+ * (PAPER.md:311).  With the paper's P0 = 2 C_o C_o^T eqs 13-14 are pairs (P0,P0),(PD,P0),(R,R) with
+ * wJ = (1/2,1,2), wK = (1/4,1/2,1), cJ = 1, cK = alpha, cLR = beta.
+ *
+ * Conventions: bohr / hartree; gradient in E_h/bohr.  Cartesian functions of a shell are ordered
+ * lx descending then ly descending (x,y,z; xx,xy,xz,yy,yz,zz; xxx,xxy,...,zzz); every contracted
+ * function is normalised to unit self-overlap (readings S7, O1).  Basis functions are
+ * numbered in shell order.
+ *
+ * All functions return 0 on success and a negative TDG_E* code on error; they never throw, abort or
+ * print.  Everything runs on the CUDA device given to tdg_create; there is NO CPU fallback
+ * (no device => TDG_ECUDA).  The context owns all memory it allocates; the caller owns every buffer it
+ * passes and may free it when the call returns.
+ */
+#ifndef TDGRAD_H
+#define TDGRAD_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDG_OK 0
+#define TDG_EINVAL (-1)        /* null pointer, non-positive count, bad shell/atom index, exponent <= 0, ... */
+#define TDG_EUNSUPPORTED (-2)  /* shell angular momentum > 3 */
+#define TDG_ENOTPLANNED (-3)   /* tdg_gradient before tdg_set_system + tdg_plan */
+#define TDG_ENOMEM (-4)        /* host or device allocation failed */
+#define TDG_ECUDA (-5)         /* CUDA runtime error; text kept in the context (tdg_last_error) */
+
+#define TDG_MAX_L 3
+#define TDG_NPAIRCLASS 10      /* (la>=lb) pair classes for l <= 3 */
+#define TDG_NCLASS 55          /* quartet classes (pair class c1 >= c2), PAPER.md:309 has 21 for l <= 2 */
+
+typedef struct tdg_ctx tdg_ctx; /* opaque */
+
+/* One contracted shell (eq 43): nprim primitives exps/coefs[prim_off .. prim_off+nprim). */
+typedef struct { int32_t atom, l, nprim, prim_off; } tdg_shell;
+
+/* Screening options (reading S9, S12). */
+typedef struct {
+  double tau;               /* threshold; <= 0: no screening                                             */
+  int32_t density_weighted; /* 0: keep quartet iff Q_ij Q_kl >= tau; 1: also Q_ij Q_kl W_ijkl >= tau      */
+  uint32_t sample_mod;      /* 0: all quartets; else keep canonical shell quartet iff hash % mod == 0     */
+  uint32_t sample_seed;
+} tdg_options;
+
+typedef struct {
+  int64_t pairs_total, pairs_kept;     /* shell pairs i>=j; those with Q_ij Q_max >= tau                  */
+  int64_t quartets_visited;            /* quartets passing the Schwarz product test                       */
+  int64_t quartets_computed;           /* ... and the density-weighted test and the subsample filter      */
+  int64_t prim_quartets;               /* primitive quartets of the computed ones                         */
+  int64_t quartets_by_class[TDG_NCLASS];
+  float ms_by_class[TDG_NCLASS];       /* CUDA-event time of each class (only when stats != NULL)         */
+  float ms_prepare;                    /* density preparation (a3)                                        */
+  float ms_total;                      /* whole tdg_gradient device time                                  */
+  int32_t launches;                    /* kernels launched by this call                                   */
+} tdg_stats;
+
+/* Create a context on CUDA device `cuda_device`.  TDG_ECUDA if there is none. */
+int tdg_create(tdg_ctx** out, int cuda_device);
+int tdg_destroy(tdg_ctx* ctx);
+
+/* Geometry and basis (HOST pointers, copied).  xyz_bohr[natom][3]; shells[nshell]; exps/coefs[nprim_total];
+ * coefs multiply NORMALISED primitives; the library normalises each contracted function (step a0).
+ * Invalidates any previous plan. */
+int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz_bohr, int nshell, const tdg_shell* shells,
+                   int nprim_total, const double* exps, const double* coefs);
+int tdg_nbf(const tdg_ctx* ctx, int* nbf);
+
+/* Steps a1-a2: shell pairs, Schwarz bounds Q_ij = sqrt(max (mn|mn)) (full operator) computed
+ * ON THE DEVICE, pair screening, sort into (la,lb,contraction degree) buckets by Q descending, work lists.
+ * Cached until tdg_set_system / tdg_plan is called again. */
+int tdg_plan(tdg_ctx* ctx, const tdg_options* opt);
+
+/* Schwarz bounds of the current system: Q[nshell][nshell] to a HOST buffer (for tests/diagnostics). */
+int tdg_schwarz(tdg_ctx* ctx, double* Q_host);
+
+/* Steps a3-a9.  A[k], B[k]: npair matrices nbf x nbf row-major FP64, ALL device pointers if
+ * `matrices_on_device` != 0, else all host pointers (copied in inside the call); never modified.
+ * wJ, wK: [npair] host.  cLR == 0 skips the long-range pass; omega > 0 required otherwise.
+ * stream: cudaStream_t (as void*) or NULL for the default stream.
+ * grad: [natom][3], device pointer if `grad_on_device` != 0 (completion is then stream-ordered) else host
+ * (the call synchronises).  Overwritten, not accumulated.  stats may be NULL (non-NULL adds per-class
+ * event timing and synchronises). */
+int tdg_gradient(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
+                 const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
+                 void* stream, double* grad, int grad_on_device, tdg_stats* stats);
+
+/* Contracted energy E (same arguments; host result) for finite-difference checks; not tuned. */
+int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
+               const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
+               void* stream, double* E_host);
+
+/* Rys roots/weights evaluator (step a5; reading S8), exposed for parity tests:
+ * for each of `count` (T[i], rho[i]) HOST inputs writes n roots x_r and n weights w_r to out[i][2n] (host),
+ * for the full operator (omega <= 0) or the attenuated one (x_r <- s^2 x_r(s^2 T), w_r <- s w_r(s^2 T),
+ * s^2 = omega^2/(omega^2+rho)).  Runs on the device.  1 <= n <= 7. */
+int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out);
+
+/* FP64 FMA throughput microbenchmark on this device (the roofline denominator; step 8d): runs chains of
+ * dependent DFMAs on all SMs for about `ms` milliseconds; writes achieved TFLOP/s (2 flop per FMA). */
+int tdg_fp64_peak(tdg_ctx* ctx, double ms, double* tflops);
+
+const char* tdg_strerror(int code);
+const char* tdg_last_error(const tdg_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
