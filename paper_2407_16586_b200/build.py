@@ -1,0 +1,63 @@
+"""Builds libtdgrad.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+    python -m paper_2407_16586_b200.build [--force]
+"""
+from __future__ import annotations
+
+import concurrent.futures as cf
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(CSRC, "build")
+LIB = os.path.join(HERE, "libtdgrad.so")
+LMAX = 3
+PAIR_CLASSES = [(la, lb) for la in range(LMAX + 1) for lb in range(la + 1)]
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
+         "-DTDG_LMAX_BUILD=%d" % LMAX]
+HEADERS = ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "../../include/tdgrad.h"]
+
+
+def _newest_header() -> float:
+    return max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
+
+
+def _compile(job):
+    src, obj, extra = job
+    cmd = [NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    return obj
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    os.makedirs(OBJ, exist_ok=True)
+    jobs = [("tdg_api.cu", os.path.join(OBJ, "tdg_api.o"), []), ("tdg_aux.cu", os.path.join(OBJ, "tdg_aux.o"), [])]
+    for la, lb in PAIR_CLASSES:
+        jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d.o" % (la, lb)), ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb]))
+    hdr = _newest_header()
+    todo = []
+    for src, obj, extra in jobs:
+        st = max(os.path.getmtime(os.path.join(CSRC, src)), hdr, os.path.getmtime(os.path.abspath(__file__)))
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < st:
+            todo.append((src, obj, extra))
+    if todo:
+        if verbose:
+            print("compiling %d objects" % len(todo), file=sys.stderr)
+        with cf.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
+            list(ex.map(_compile, todo))
+    objs = [j[1] for j in jobs]
+    if todo or not os.path.exists(LIB):
+        cmd = [NVCC, "-shared", "-o", LIB] + objs
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("link failed:\n%s\n%s" % (r.stdout, r.stderr))
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose=True))

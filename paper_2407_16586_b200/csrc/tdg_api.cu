@@ -1,0 +1,511 @@
+// tdg_api.cu — C ABI of libtdgrad (include/tdgrad.h): context, host planner (steps a0-a2), density preparation
+// and per-class launches (a3-a9).  No CPU arithmetic fallback: all integrals are evaluated by the CUDA kernels.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/tdgrad.h"
+#include "tdg_grad.cuh"
+#include "tdg_internal.h"
+
+#define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
+
+tdg_launch_fn tdg_class_launcher_00(int, int);
+tdg_launch_fn tdg_class_launcher_10(int, int);
+tdg_launch_fn tdg_class_launcher_11(int, int);
+tdg_launch_fn tdg_class_launcher_20(int, int);
+tdg_launch_fn tdg_class_launcher_21(int, int);
+tdg_launch_fn tdg_class_launcher_22(int, int);
+#if TDG_LMAX_BUILD >= 3
+tdg_launch_fn tdg_class_launcher_30(int, int);
+tdg_launch_fn tdg_class_launcher_31(int, int);
+tdg_launch_fn tdg_class_launcher_32(int, int);
+tdg_launch_fn tdg_class_launcher_33(int, int);
+#endif
+
+tdg_launch_fn tdg_get_launcher(int la, int lb, int lc, int ld) {
+  switch (PCLS(la, lb)) {
+    case 0: return tdg_class_launcher_00(lc, ld);
+    case 1: return tdg_class_launcher_10(lc, ld);
+    case 2: return tdg_class_launcher_11(lc, ld);
+    case 3: return tdg_class_launcher_20(lc, ld);
+    case 4: return tdg_class_launcher_21(lc, ld);
+    case 5: return tdg_class_launcher_22(lc, ld);
+#if TDG_LMAX_BUILD >= 3
+    case 6: return tdg_class_launcher_30(lc, ld);
+    case 7: return tdg_class_launcher_31(lc, ld);
+    case 8: return tdg_class_launcher_32(lc, ld);
+    case 9: return tdg_class_launcher_33(lc, ld);
+#endif
+  }
+  return nullptr;
+}
+
+namespace {
+
+struct Bucket {       // shell pairs of one (la, lb, primitive-pair count), sorted by Q descending
+  int la, lb, npp, n;
+  PairHdr* d_hdr = nullptr;
+  double* d_prim = nullptr;
+  std::vector<double> Q;   // host copy of the sorted bounds
+  std::vector<int> last_same;  // unused
+};
+struct Work {         // one kernel launch: bra bucket x ket bucket
+  int b1, b2, cls, nblocks, ntiles;
+  int* d_cum = nullptr;
+};
+
+}  // namespace
+
+struct tdg_ctx {
+  int device = 0;
+  std::string err;
+  // system
+  int natom = 0, nshell = 0, nprim = 0, nbf = 0;
+  std::vector<double> xyz, exps, cn;   // cn: contraction coefficient x primitive radial norm x shell norm (a0)
+  std::vector<DevShell> shells;
+  double *d_xyz = nullptr, *d_exps = nullptr, *d_cn = nullptr, *d_Q = nullptr, *d_rys = nullptr;
+  DevShell* d_shells = nullptr;
+  bool have_Q = false;
+  // plan
+  bool planned = false;
+  tdg_options opt{};
+  std::vector<Bucket> buckets;
+  std::vector<Work> work;
+  int64_t pairs_total = 0, pairs_kept = 0;
+  // per-call scratch
+  double* d_grad = nullptr;
+  double* d_dmax = nullptr;
+  unsigned long long* d_counters = nullptr;   // [nwork][3]
+  size_t counters_cap = 0;
+  std::vector<std::pair<size_t, void*>> scratch;  // cached matrix-sized buffers (bytes, ptr)
+  std::vector<bool> scratch_used;
+};
+
+static int fail_cuda(tdg_ctx* c, cudaError_t e, const char* where) {
+  c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? TDG_ENOMEM : TDG_ECUDA;
+}
+#define CK(call)                                                  \
+  do {                                                            \
+    cudaError_t e_ = (call);                                      \
+    if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);      \
+  } while (0)
+
+static void free_plan(tdg_ctx* c) {
+  for (auto& b : c->buckets) { cudaFree(b.d_hdr); cudaFree(b.d_prim); }
+  for (auto& w : c->work) cudaFree(w.d_cum);
+  c->buckets.clear(); c->work.clear();
+  c->planned = false;
+}
+static void free_system(tdg_ctx* c) {
+  free_plan(c);
+  cudaFree(c->d_xyz); cudaFree(c->d_exps); cudaFree(c->d_cn); cudaFree(c->d_Q); cudaFree(c->d_shells);
+  cudaFree(c->d_grad); cudaFree(c->d_dmax);
+  c->d_xyz = c->d_exps = c->d_cn = c->d_Q = c->d_grad = c->d_dmax = nullptr; c->d_shells = nullptr;
+  for (auto& s : c->scratch) cudaFree(s.second);
+  c->scratch.clear(); c->scratch_used.clear();
+  c->have_Q = false; c->nshell = 0;
+}
+
+extern "C" const char* tdg_strerror(int code) {
+  switch (code) {
+    case TDG_OK: return "ok";
+    case TDG_EINVAL: return "invalid argument";
+    case TDG_EUNSUPPORTED: return "unsupported (angular momentum > 3 or class not built)";
+    case TDG_ENOTPLANNED: return "tdg_set_system/tdg_plan not called";
+    case TDG_ENOMEM: return "out of memory";
+    case TDG_ECUDA: return "CUDA error";
+  }
+  return "unknown error";
+}
+extern "C" const char* tdg_last_error(const tdg_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+extern "C" int tdg_create(tdg_ctx** out, int cuda_device) {
+  if (!out) return TDG_EINVAL;
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) { cudaGetLastError(); return TDG_ECUDA; }
+  if (cudaSetDevice(cuda_device) != cudaSuccess) return TDG_ECUDA;
+  tdg_ctx* ctx = new (std::nothrow) tdg_ctx();
+  if (!ctx) return TDG_ENOMEM;
+  ctx->device = cuda_device;
+  if (tdg_upload_rys_table(&ctx->d_rys) != cudaSuccess) { delete ctx; return TDG_ECUDA; }
+  *out = ctx;
+  return TDG_OK;
+}
+
+extern "C" int tdg_destroy(tdg_ctx* ctx) {
+  if (!ctx) return TDG_EINVAL;
+  cudaSetDevice(ctx->device);
+  free_system(ctx);
+  cudaFree(ctx->d_rys); cudaFree(ctx->d_counters);
+  delete ctx;
+  return TDG_OK;
+}
+
+extern "C" int tdg_nbf(const tdg_ctx* ctx, int* nbf) {
+  if (!ctx || !nbf) return TDG_EINVAL;
+  *nbf = ctx->nbf;
+  return TDG_OK;
+}
+
+// Step a0 (eq 38 "N"; eq 43; O1): coefficient of each primitive =
+// d_k (2z/pi)^(3/4) (4z)^(l/2) / sqrt(S), S = sum_kk' d_k d_k' (2 sqrt(z z')/(z+z'))^(l+3/2); the per-component
+// factor 1/sqrt((2lx-1)!!(2ly-1)!!(2lz-1)!!) is applied to the density products inside the kernels.
+extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int nshell, const tdg_shell* shells,
+                              int nprim_total, const double* exps, const double* coefs) {
+  if (!ctx) return TDG_EINVAL;
+  if (!xyz || !shells || !exps || !coefs || natom <= 0 || nshell <= 0 || nprim_total <= 0) return TDG_EINVAL;
+  for (int s = 0; s < nshell; ++s) {
+    const tdg_shell& sh = shells[s];
+    if (sh.atom < 0 || sh.atom >= natom || sh.nprim <= 0 || sh.prim_off < 0 || sh.prim_off + sh.nprim > nprim_total || sh.l < 0) return TDG_EINVAL;
+    if (sh.l > TDG_MAX_L || sh.l > TDG_LMAX_BUILD) return TDG_EUNSUPPORTED;
+    for (int k = 0; k < sh.nprim; ++k) if (!(exps[sh.prim_off + k] > 0.0)) return TDG_EINVAL;
+  }
+  cudaSetDevice(ctx->device);
+  free_system(ctx);
+  ctx->natom = natom; ctx->nshell = nshell; ctx->nprim = nprim_total;
+  ctx->xyz.assign(xyz, xyz + 3 * (size_t)natom);
+  ctx->exps.assign(exps, exps + nprim_total);
+  ctx->cn.assign(nprim_total, 0.0);
+  ctx->shells.resize(nshell);
+  int off = 0;
+  const double PI = 3.14159265358979323846;
+  for (int s = 0; s < nshell; ++s) {
+    const tdg_shell& sh = shells[s];
+    double S = 0.0;
+    for (int k = 0; k < sh.nprim; ++k)
+      for (int k2 = 0; k2 < sh.nprim; ++k2) {
+        const double z1 = exps[sh.prim_off + k], z2 = exps[sh.prim_off + k2];
+        S += coefs[sh.prim_off + k] * coefs[sh.prim_off + k2] * std::pow(2.0 * std::sqrt(z1 * z2) / (z1 + z2), sh.l + 1.5);
+      }
+    if (!(S > 0.0)) return TDG_EINVAL;
+    for (int k = 0; k < sh.nprim; ++k) {
+      const double z = exps[sh.prim_off + k];
+      ctx->cn[sh.prim_off + k] = coefs[sh.prim_off + k] * std::pow(2.0 * z / PI, 0.75) * std::pow(4.0 * z, 0.5 * sh.l) / std::sqrt(S);
+    }
+    ctx->shells[s] = DevShell{sh.atom, sh.l, sh.nprim, sh.prim_off, off, 0};
+    off += ncart(sh.l);
+  }
+  ctx->nbf = off;
+  CK(cudaMalloc(&ctx->d_xyz, sizeof(double) * 3 * natom));
+  CK(cudaMalloc(&ctx->d_exps, sizeof(double) * nprim_total));
+  CK(cudaMalloc(&ctx->d_cn, sizeof(double) * nprim_total));
+  CK(cudaMalloc(&ctx->d_shells, sizeof(DevShell) * nshell));
+  CK(cudaMalloc(&ctx->d_Q, sizeof(double) * (size_t)nshell * nshell));
+  CK(cudaMalloc(&ctx->d_grad, sizeof(double) * 3 * natom));
+  CK(cudaMemcpy(ctx->d_xyz, ctx->xyz.data(), sizeof(double) * 3 * natom, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(ctx->d_exps, ctx->exps.data(), sizeof(double) * nprim_total, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(ctx->d_cn, ctx->cn.data(), sizeof(double) * nprim_total, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(ctx->d_shells, ctx->shells.data(), sizeof(DevShell) * nshell, cudaMemcpyHostToDevice));
+  return TDG_OK;
+}
+
+static int ensure_schwarz(tdg_ctx* ctx) {
+  if (ctx->have_Q) return TDG_OK;
+  CK(tdg_launch_schwarz(ctx->d_shells, ctx->nshell, ctx->d_xyz, ctx->d_exps, ctx->d_cn, ctx->d_rys, ctx->d_Q, 0));
+  CK(cudaDeviceSynchronize());
+  ctx->have_Q = true;
+  return TDG_OK;
+}
+
+extern "C" int tdg_schwarz(tdg_ctx* ctx, double* Q_host) {
+  if (!ctx || !Q_host) return TDG_EINVAL;
+  if (ctx->nshell <= 0) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  int rc = ensure_schwarz(ctx);
+  if (rc) return rc;
+  CK(cudaMemcpy(Q_host, ctx->d_Q, sizeof(double) * (size_t)ctx->nshell * ctx->nshell, cudaMemcpyDeviceToHost));
+  return TDG_OK;
+}
+
+// Steps a1-a2.
+extern "C" int tdg_plan(tdg_ctx* ctx, const tdg_options* opt) {
+  if (!ctx) return TDG_EINVAL;
+  if (ctx->nshell <= 0) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  free_plan(ctx);
+  ctx->opt = opt ? *opt : tdg_options{0.0, 0, 0, 0};
+  const double tau = ctx->opt.tau;
+  const int ns = ctx->nshell;
+  std::vector<double> Q;
+  double Qmax = 0.0;
+  if (tau > 0.0) {
+    int rc = ensure_schwarz(ctx);
+    if (rc) return rc;
+    try { Q.resize((size_t)ns * ns); } catch (...) { return TDG_ENOMEM; }
+    CK(cudaMemcpy(Q.data(), ctx->d_Q, sizeof(double) * Q.size(), cudaMemcpyDeviceToHost));
+    for (double q : Q) if (q > Qmax) Qmax = q;
+  }
+  struct HP { int i, j; double Q; };
+  std::map<std::tuple<int, int, int>, std::vector<HP>> groups;  // (pair class, npp) -> pairs; ordered
+  ctx->pairs_total = (int64_t)ns * (ns + 1) / 2;
+  ctx->pairs_kept = 0;
+  for (int i = 0; i < ns; ++i)
+    for (int j = 0; j <= i; ++j) {
+      double q = 1.0;
+      if (tau > 0.0) { q = Q[(size_t)i * ns + j]; if (!(q * Qmax >= tau)) continue; }
+      int a = i, b = j;   // orient: higher l first; ties keep i (the larger index) first
+      if (ctx->shells[a].l < ctx->shells[b].l) std::swap(a, b);
+      const int la = ctx->shells[a].l, lb = ctx->shells[b].l;
+      groups[std::make_tuple(PCLS(la, lb), ctx->shells[a].nprim * ctx->shells[b].nprim, 0)].push_back(HP{a, b, q});
+      ++ctx->pairs_kept;
+    }
+  try {
+    for (auto& kv : groups) {
+      auto& v = kv.second;
+      std::sort(v.begin(), v.end(), [](const HP& x, const HP& y) {
+        if (x.Q != y.Q) return x.Q > y.Q;
+        if (x.i != y.i) return x.i < y.i;
+        return x.j < y.j;
+      });
+      Bucket B;
+      B.la = ctx->shells[v[0].i].l; B.lb = ctx->shells[v[0].j].l; B.npp = std::get<1>(kv.first); B.n = (int)v.size();
+      std::vector<PairHdr> hdr(v.size());
+      std::vector<double> prim(v.size() * (size_t)B.npp * TDG_PRIM_STRIDE, 0.0);
+      B.Q.resize(v.size());
+      for (size_t t = 0; t < v.size(); ++t) {
+        const DevShell& sa = ctx->shells[v[t].i]; const DevShell& sb = ctx->shells[v[t].j];
+        const double* A = &ctx->xyz[3 * sa.atom]; const double* Bc = &ctx->xyz[3 * sb.atom];
+        PairHdr& h = hdr[t];
+        double R2 = 0.0;
+        for (int d = 0; d < 3; ++d) { h.A[d] = A[d]; h.AB[d] = A[d] - Bc[d]; R2 += h.AB[d] * h.AB[d]; }
+        h.Q = v[t].Q; h.ish = v[t].i; h.jsh = v[t].j; h.atomA = sa.atom; h.atomB = sb.atom; h.offA = sa.bf_off; h.offB = sb.bf_off;
+        B.Q[t] = v[t].Q;
+        double* pp = &prim[t * (size_t)B.npp * TDG_PRIM_STRIDE];
+        for (int ka = 0; ka < sa.nprim; ++ka)
+          for (int kb = 0; kb < sb.nprim; ++kb) {
+            const double a = ctx->exps[sa.prim_off + ka], b = ctx->exps[sb.prim_off + kb], p = a + b;
+            double* r = pp + (size_t)(ka * sb.nprim + kb) * TDG_PRIM_STRIDE;
+            r[0] = p;
+            for (int d = 0; d < 3; ++d) r[1 + d] = (a * A[d] + b * Bc[d]) / p;
+            r[4] = ctx->cn[sa.prim_off + ka] * ctx->cn[sb.prim_off + kb] * std::exp(-a * b / p * R2);
+            r[5] = a; r[6] = b; r[7] = 0.0;
+          }
+      }
+      CK(cudaMalloc(&B.d_hdr, sizeof(PairHdr) * hdr.size()));
+      CK(cudaMalloc(&B.d_prim, sizeof(double) * prim.size()));
+      CK(cudaMemcpy(B.d_hdr, hdr.data(), sizeof(PairHdr) * hdr.size(), cudaMemcpyHostToDevice));
+      CK(cudaMemcpy(B.d_prim, prim.data(), sizeof(double) * prim.size(), cudaMemcpyHostToDevice));
+      ctx->buckets.push_back(std::move(B));
+    }
+    // work lists: bucket b1 >= b2 (bucket order = (pair class, npp) ascending, so bra class >= ket class)
+    const int nb = (int)ctx->buckets.size();
+    for (int b1 = 0; b1 < nb; ++b1)
+      for (int b2 = 0; b2 <= b1; ++b2) {
+        const Bucket& X = ctx->buckets[b1]; const Bucket& Y = ctx->buckets[b2];
+        const int ntiles = (X.n + TDG_WARP - 1) / TDG_WARP;
+        std::vector<int> cum(ntiles + 1, 0);
+        for (int t = 0; t < ntiles; ++t) {
+          int klen = Y.n;
+          if (tau > 0.0) {   // kets with Q_bra0 * Q_ket >= tau form a prefix (sorted descending)
+            const double qb = X.Q[(size_t)t * TDG_WARP];
+            klen = (int)(std::partition_point(Y.Q.begin(), Y.Q.end(), [&](double qk) { return qb * qk >= tau; }) - Y.Q.begin());
+          }
+          if (b1 == b2) klen = std::min(klen, std::min(X.n, (t + 1) * TDG_WARP));
+          cum[t + 1] = cum[t] + (klen + TDG_KB - 1) / TDG_KB;
+        }
+        if (cum[ntiles] == 0) continue;
+        Work W;
+        W.b1 = b1; W.b2 = b2; W.ntiles = ntiles; W.nblocks = cum[ntiles];
+        const int c1 = PCLS(X.la, X.lb), c2 = PCLS(Y.la, Y.lb);
+        W.cls = c1 * (c1 + 1) / 2 + c2;
+        CK(cudaMalloc(&W.d_cum, sizeof(int) * cum.size()));
+        CK(cudaMemcpy(W.d_cum, cum.data(), sizeof(int) * cum.size(), cudaMemcpyHostToDevice));
+        ctx->work.push_back(W);
+      }
+  } catch (const std::bad_alloc&) { free_plan(ctx); return TDG_ENOMEM; }
+  const size_t need = ctx->work.size() * 3 + 3;
+  if (need > ctx->counters_cap) {
+    cudaFree(ctx->d_counters); ctx->d_counters = nullptr;
+    CK(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * need));
+    ctx->counters_cap = need;
+  }
+  ctx->planned = true;
+  return TDG_OK;
+}
+
+// ---- per-call density preparation (a3) ----
+static void* scratch_get(tdg_ctx* ctx, size_t bytes) {
+  for (size_t i = 0; i < ctx->scratch.size(); ++i)
+    if (!ctx->scratch_used[i] && ctx->scratch[i].first == bytes) { ctx->scratch_used[i] = true; return ctx->scratch[i].second; }
+  void* p = nullptr;
+  if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  ctx->scratch.push_back({bytes, p}); ctx->scratch_used.push_back(true);
+  return p;
+}
+
+namespace {
+struct Canon { const double* S; const double* N; };   // symmetric / antisymmetric parts (N == nullptr: symmetric input)
+}
+
+static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int on_dev,
+                           const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
+                           cudaStream_t st, tdg_stats* stats) {
+  const int n = ctx->nbf;
+  const size_t mbytes = sizeof(double) * (size_t)n * n;
+  std::fill(ctx->scratch_used.begin(), ctx->scratch_used.end(), false);
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
+  if (stats) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventCreate(&ev2); cudaEventRecord(ev0, st); }
+  // unique input matrices -> device pointers
+  std::map<const double*, const double*> dev;   // input pointer -> device pointer
+  for (int k = 0; k < npair; ++k)
+    for (const double* M : {A[k], B[k]}) {
+      if (dev.count(M)) continue;
+      if (on_dev) dev[M] = M;
+      else {
+        double* d = (double*)scratch_get(ctx, mbytes);
+        if (!d) { ctx->err = "device allocation of a density matrix failed"; return TDG_ENOMEM; }
+        CK(cudaMemcpyAsync(d, M, mbytes, cudaMemcpyHostToDevice, st));
+        dev[M] = d;
+      }
+    }
+  // symmetric / antisymmetric split (K(A,B) = K(As,Bs) + K(An,Bn) after 8-fold symmetrisation)
+  std::map<const double*, Canon> canon;
+  {
+    double* d_as = (double*)scratch_get(ctx, 256);
+    if (!d_as) return TDG_ENOMEM;
+    std::vector<const double*> keys;
+    for (auto& kv : dev) keys.push_back(kv.first);
+    if (keys.size() > 32) return TDG_EINVAL;
+    CK(cudaMemsetAsync(d_as, 0, 256, st));
+    for (size_t i = 0; i < keys.size(); ++i) CK(tdg_launch_asym(dev[keys[i]], n, d_as + i, st));
+    double as[32];
+    CK(cudaMemcpyAsync(as, d_as, sizeof(double) * keys.size(), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    for (size_t i = 0; i < keys.size(); ++i) {
+      if (as[i] == 0.0) canon[keys[i]] = Canon{dev[keys[i]], nullptr};
+      else {
+        double* S = (double*)scratch_get(ctx, mbytes); double* N = (double*)scratch_get(ctx, mbytes);
+        if (!S || !N) { ctx->err = "device allocation of symmetrised densities failed"; return TDG_ENOMEM; }
+        CK(tdg_launch_symsplit(dev[keys[i]], n, S, N, st));
+        canon[keys[i]] = Canon{S, N};
+      }
+    }
+  }
+  KParams P{};
+  P.nJ = 0; P.nK = 0;
+  double CJ = 0.0, CKs = 0.0;
+  for (int k = 0; k < npair; ++k) {
+    const Canon& a = canon[A[k]]; const Canon& b = canon[B[k]];
+    CJ += std::fabs(wJ[k] * cJ); CKs += std::fabs(wK[k]);
+    if (wJ[k] * cJ != 0.0) {
+      if (P.nJ >= TDG_MAXP) return TDG_EINVAL;
+      P.jp[P.nJ++] = DensPair{a.S, b.S, 4.0 * wJ[k] * cJ};
+    }
+    if (wK[k] != 0.0 && (cK != 0.0 || cLR != 0.0)) {
+      if (P.nK + 2 > TDG_MAXP) return TDG_EINVAL;
+      P.kp[P.nK++] = DensPair{a.S, b.S, -2.0 * wK[k]};
+      if (a.N && b.N) P.kp[P.nK++] = DensPair{a.N, b.N, -2.0 * wK[k]};
+    }
+  }
+  CKs *= std::fabs(cK) + std::fabs(cLR);
+  P.CJ = CJ; P.CK = CKs;
+  P.tau = ctx->opt.tau; P.density_weighted = (ctx->opt.tau > 0.0) ? ctx->opt.density_weighted : 0;
+  P.nshell = ctx->nshell; P.sample_mod = ctx->opt.sample_mod; P.sample_seed = ctx->opt.sample_seed;
+  P.nbf = n; P.cK = cK; P.cLR = cLR; P.omega2 = omega * omega; P.use_lr = (cLR != 0.0) ? 1 : 0;
+  P.grad = ctx->d_grad; P.rys_tab = ctx->d_rys;
+  if (P.density_weighted) {   // d_ij over ALL input matrices (reading S9)
+    if (!ctx->d_dmax) CK(cudaMalloc(&ctx->d_dmax, sizeof(double) * (size_t)ctx->nshell * ctx->nshell));
+    std::vector<const double*> mats;
+    for (auto& kv : dev) mats.push_back(kv.second);
+    const double** d_list = (const double**)scratch_get(ctx, 512);
+    if (!d_list) return TDG_ENOMEM;
+    CK(cudaMemcpyAsync(d_list, mats.data(), sizeof(double*) * mats.size(), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));   // mats is a local vector
+    CK(tdg_launch_dmax(d_list, (int)mats.size(), n, ctx->d_shells, ctx->nshell, ctx->d_dmax, st));
+    P.dmax = ctx->d_dmax;
+  }
+  CK(cudaMemsetAsync(ctx->d_grad, 0, sizeof(double) * 3 * ctx->natom, st));
+  CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * (ctx->work.size() * 3 + 3), st));
+  if (stats) cudaEventRecord(ev1, st);
+  int launches = 0;
+  std::vector<cudaEvent_t> evs;
+  for (size_t w = 0; w < ctx->work.size(); ++w) {
+    const Work& W = ctx->work[w];
+    const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
+    tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb);
+    if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+    P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
+    P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
+    P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
+    P.counters = ctx->d_counters + 3 * w;
+    if (stats) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); evs.push_back(e); }
+    fn(P, W.nblocks, st);
+    ++launches;
+  }
+  CK(cudaGetLastError());
+  if (stats) {
+    cudaEventRecord(ev2, st);
+    CK(cudaStreamSynchronize(st));
+    std::vector<unsigned long long> cnt(ctx->work.size() * 3 + 3);
+    CK(cudaMemcpy(cnt.data(), ctx->d_counters, sizeof(unsigned long long) * cnt.size(), cudaMemcpyDeviceToHost));
+    std::memset(stats, 0, sizeof(*stats));
+    stats->pairs_total = ctx->pairs_total; stats->pairs_kept = ctx->pairs_kept;
+    for (size_t w = 0; w < ctx->work.size(); ++w) {
+      stats->quartets_visited += (int64_t)cnt[3 * w]; stats->quartets_computed += (int64_t)cnt[3 * w + 1];
+      stats->prim_quartets += (int64_t)cnt[3 * w + 2];
+      stats->quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 1];
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, evs[w], w + 1 < evs.size() ? evs[w + 1] : ev2);
+      stats->ms_by_class[ctx->work[w].cls] += ms;
+    }
+    cudaEventElapsedTime(&stats->ms_prepare, ev0, ev1);
+    cudaEventElapsedTime(&stats->ms_total, ev0, ev2);
+    stats->launches = launches + (int)dev.size() + (P.density_weighted ? 2 : 0);
+    for (auto e : evs) cudaEventDestroy(e);
+    cudaEventDestroy(ev0); cudaEventDestroy(ev1); cudaEventDestroy(ev2);
+  }
+  return TDG_OK;
+}
+
+extern "C" int tdg_gradient(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
+                            const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
+                            void* stream, double* grad, int grad_on_device, tdg_stats* stats) {
+  if (!ctx) return TDG_EINVAL;
+  if (!A || !B || !wJ || !wK || !grad || npair <= 0 || npair > TDG_MAXP) return TDG_EINVAL;
+  for (int k = 0; k < npair; ++k) if (!A[k] || !B[k]) return TDG_EINVAL;
+  if (cLR != 0.0 && !(omega > 0.0)) return TDG_EINVAL;
+  if (!ctx->planned) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = run_contraction(ctx, npair, A, B, matrices_on_device, wJ, wK, cJ, cK, cLR, omega, st, stats);
+  if (rc) return rc;
+  const size_t gb = sizeof(double) * 3 * ctx->natom;
+  if (grad_on_device) CK(cudaMemcpyAsync(grad, ctx->d_grad, gb, cudaMemcpyDeviceToDevice, st));
+  else { CK(cudaMemcpyAsync(grad, ctx->d_grad, gb, cudaMemcpyDeviceToHost, st)); CK(cudaStreamSynchronize(st)); }
+  return TDG_OK;
+}
+
+extern "C" int tdg_energy(tdg_ctx* ctx, int, const double* const*, const double* const*, int, const double*, const double*,
+                          double, double, double, double, void*, double*) {
+  if (!ctx) return TDG_EINVAL;
+  ctx->err = "tdg_energy: not built in this round";
+  return TDG_EUNSUPPORTED;
+}
+
+extern "C" int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out) {
+  if (!ctx || !T || !rho || !out || n < 1 || n > 7 || count <= 0) return TDG_EINVAL;
+  cudaSetDevice(ctx->device);
+  double *dT = nullptr, *dr = nullptr, *dout = nullptr;
+  CK(cudaMalloc(&dT, sizeof(double) * count)); CK(cudaMalloc(&dr, sizeof(double) * count));
+  CK(cudaMalloc(&dout, sizeof(double) * (size_t)count * 2 * n));
+  CK(cudaMemcpy(dT, T, sizeof(double) * count, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(dr, rho, sizeof(double) * count, cudaMemcpyHostToDevice));
+  CK(tdg_launch_rys(n, count, dT, dr, omega, ctx->d_rys, dout, 0));
+  CK(cudaMemcpy(out, dout, sizeof(double) * (size_t)count * 2 * n, cudaMemcpyDeviceToHost));
+  cudaFree(dT); cudaFree(dr); cudaFree(dout);
+  return TDG_OK;
+}
+
+extern "C" int tdg_fp64_peak(tdg_ctx* ctx, double ms, double* tflops) {
+  if (!ctx || !tflops) return TDG_EINVAL;
+  cudaSetDevice(ctx->device);
+  CK(tdg_run_fp64_peak(ms, tflops));
+  return TDG_OK;
+}

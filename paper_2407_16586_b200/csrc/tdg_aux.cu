@@ -1,0 +1,300 @@
+// tdg_aux.cu — auxiliary device kernels of libtdgrad: Schwarz bounds (a1), density preparation (a3), the Rys
+// evaluator exposed for tests (a5) and the FP64 FMA microbenchmark (roofline denominator).
+#include "tdg_common.cuh"
+#include "tdg_internal.h"
+#include "rys_tables.inc"
+
+cudaError_t tdg_upload_rys_table(double** d_tab) {
+  cudaError_t e = cudaMalloc(d_tab, sizeof(RYS_TAB));
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*d_tab, RYS_TAB, sizeof(RYS_TAB), cudaMemcpyHostToDevice);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Runtime-l plain 2-D integrals (no raising): I[i][j][k][l], i<=la, j<=lb, k<=lc, l<=ld, each dimension 4.
+__device__ static void build2d_rt(int la, int lb, int lc, int ld, double c00, double c00p, double b00, double b10,
+                                  double b01, double ab, double cd, double v00, double* I) {
+  const int nmx = la + lb, mmx = lc + ld;
+  double V[7][7];
+  V[0][0] = v00;
+  for (int n = 0; n < nmx; ++n) V[n + 1][0] = c00 * V[n][0] + (n > 0 ? n * b10 * V[n - 1][0] : 0.0);
+  for (int m = 0; m < mmx; ++m)
+    for (int n = 0; n <= nmx; ++n) {
+      double v = c00p * V[n][m];
+      if (m > 0) v += m * b01 * V[n][m - 1];
+      if (n > 0) v += n * b00 * V[n - 1][m];
+      V[n][m + 1] = v;
+    }
+  double W[4][4][7];
+  for (int m = 0; m <= mmx; ++m) {
+    double h[7];
+    for (int i = 0; i <= nmx; ++i) h[i] = V[i][m];
+    for (int j = 0; j <= lb; ++j) {
+      for (int i = 0; i <= la; ++i) W[i][j][m] = h[i];
+      for (int i = 0; i + j < nmx; ++i) h[i] = h[i + 1] + ab * h[i];
+    }
+  }
+  for (int i = 0; i <= la; ++i)
+    for (int j = 0; j <= lb; ++j) {
+      double g[7];
+      for (int k = 0; k <= mmx; ++k) g[k] = W[i][j][k];
+      for (int l = 0; l <= ld; ++l) {
+        for (int k = 0; k <= lc; ++k) I[((i * 4 + j) * 4 + k) * 4 + l] = g[k];
+        for (int k = 0; k + l < mmx; ++k) g[k] = g[k + 1] + cd * g[k];
+      }
+    }
+}
+
+__device__ static void rys_roots_rt(int n, const double* tab, double T, double* x, double* w) {
+  switch (n) {
+    case 1: rys_roots<1>(tab, T, x, w); break;
+    case 2: rys_roots<2>(tab, T, x, w); break;
+    case 3: rys_roots<3>(tab, T, x, w); break;
+    case 4: rys_roots<4>(tab, T, x, w); break;
+    case 5: rys_roots<5>(tab, T, x, w); break;
+    case 6: rys_roots<6>(tab, T, x, w); break;
+    default: rys_roots<7>(tab, T, x, w); break;
+  }
+}
+
+// One thread per shell pair i >= j: Q_ij = sqrt(max_{mn} (mn|mn)) with the full 1/r operator.
+__global__ void schwarz_kernel(const DevShell* __restrict__ sh, int ns, const double* __restrict__ xyz,
+                               const double* __restrict__ exps, const double* __restrict__ cn,
+                               const double* __restrict__ tab, double* __restrict__ Q) {
+  const int i = blockIdx.y, j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j > i || j >= ns) return;
+  DevShell si = sh[i], sj = sh[j];
+  if (si.l < sj.l) { DevShell t = si; si = sj; sj = t; }
+  const int la = si.l, lb = sj.l;
+  const double Ax = xyz[3 * si.atom], Ay = xyz[3 * si.atom + 1], Az = xyz[3 * si.atom + 2];
+  const double ABx = Ax - xyz[3 * sj.atom], ABy = Ay - xyz[3 * sj.atom + 1], ABz = Az - xyz[3 * sj.atom + 2];
+  const double R2 = ABx * ABx + ABy * ABy + ABz * ABz;
+  // cheap exit: every primitive-pair prefactor negligible => Q is far below any threshold
+  double kmax = 0.0;
+  for (int a = 0; a < si.nprim; ++a)
+    for (int b = 0; b < sj.nprim; ++b) {
+      const double ea = exps[si.prim_off + a], eb = exps[sj.prim_off + b];
+      const double k = fabs(cn[si.prim_off + a] * cn[sj.prim_off + b]) * exp(-ea * eb / (ea + eb) * R2);
+      if (k > kmax) kmax = k;
+    }
+  if (kmax < 1e-30) { Q[(size_t)i * ns + j] = 0.0; Q[(size_t)j * ns + i] = 0.0; return; }
+  const int na = ncart(la), nb = ncart(lb);
+  const int nr = (la + lb) + 1;  // floor(2(la+lb)/2)+1 roots for a plain ERI of total L = 2(la+lb)
+  double diag[100];
+  for (int t = 0; t < na * nb; ++t) diag[t] = 0.0;
+  double Ix[256], Iy[256], Iz[256];
+  for (int a = 0; a < si.nprim; ++a)
+    for (int b = 0; b < sj.nprim; ++b) {
+      const double ea = exps[si.prim_off + a], eb = exps[sj.prim_off + b];
+      const double p = ea + eb, Kab = cn[si.prim_off + a] * cn[sj.prim_off + b] * exp(-ea * eb / p * R2);
+      if (fabs(Kab) < 1e-30 * kmax) continue;
+      const double PAx = -eb / p * ABx, PAy = -eb / p * ABy, PAz = -eb / p * ABz;  // P - A
+      for (int c = 0; c < si.nprim; ++c)
+        for (int d = 0; d < sj.nprim; ++d) {
+          const double ec = exps[si.prim_off + c], ed = exps[sj.prim_off + d];
+          const double q = ec + ed, Kcd = cn[si.prim_off + c] * cn[sj.prim_off + d] * exp(-ec * ed / q * R2);
+          if (fabs(Kcd) < 1e-30 * kmax) continue;
+          const double QCx = -ed / q * ABx, QCy = -ed / q * ABy, QCz = -ed / q * ABz;  // Q - C, C = A
+          const double PQx = PAx - QCx, PQy = PAy - QCy, PQz = PAz - QCz;
+          const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+          const double T = rho * (PQx * PQx + PQy * PQy + PQz * PQz);
+          const double pref = 34.986836655249725693 * Kab * Kcd * rpq * sqrt(rpq) / rho;
+          double xr[7], wr[7];
+          rys_roots_rt(nr, tab, T, xr, wr);
+          for (int r = 0; r < nr; ++r) {
+            const double x = xr[r], w = wr[r] * pref;
+            const double b00 = 0.5 * x * rpq, b10 = (0.5 - q * b00) / p, b01 = (0.5 - p * b00) / q;
+            const double fq = q * rpq * x, fp = p * rpq * x;
+            build2d_rt(la, lb, la, lb, PAx - fq * PQx, QCx + fp * PQx, b00, b10, b01, ABx, ABx, 1.0, Ix);
+            build2d_rt(la, lb, la, lb, PAy - fq * PQy, QCy + fp * PQy, b00, b10, b01, ABy, ABy, 1.0, Iy);
+            build2d_rt(la, lb, la, lb, PAz - fq * PQz, QCz + fp * PQz, b00, b10, b01, ABz, ABz, w, Iz);
+            for (int m = 0; m < na; ++m) {
+              const unsigned va = c_cart[la][m];
+              const int ax = va & 15, ay = (va >> 4) & 15, az = (va >> 8) & 15;
+              for (int n = 0; n < nb; ++n) {
+                const unsigned vb = c_cart[lb][n];
+                const int bx = vb & 15, by = (vb >> 4) & 15, bz = (vb >> 8) & 15;
+                diag[m * nb + n] += Ix[((ax * 4 + bx) * 4 + ax) * 4 + bx] * Iy[((ay * 4 + by) * 4 + ay) * 4 + by] *
+                                    Iz[((az * 4 + bz) * 4 + az) * 4 + bz];
+              }
+            }
+          }
+        }
+    }
+  double mx = 0.0;
+  for (int m = 0; m < na; ++m)
+    for (int n = 0; n < nb; ++n) {
+      const double cc = c_cnorm[la][m] * c_cnorm[lb][n];
+      const double v = diag[m * nb + n] * cc * cc;
+      if (v > mx) mx = v;
+    }
+  const double q = sqrt(mx);
+  Q[(size_t)i * ns + j] = q;
+  Q[(size_t)j * ns + i] = q;
+}
+
+cudaError_t tdg_launch_schwarz(const DevShell* sh, int ns, const double* xyz, const double* exps, const double* cn,
+                               const double* rys_tab, double* Q, cudaStream_t s) {
+  dim3 block(64), grid((ns + 63) / 64, ns);
+  schwarz_kernel<<<grid, block, 0, s>>>(sh, ns, xyz, exps, cn, rys_tab, Q);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Density preparation (a3)
+__device__ __forceinline__ void atomic_max_nonneg(double* addr, double v) {
+  atomicMax((unsigned long long*)addr, (unsigned long long)__double_as_longlong(v));
+}
+
+__global__ void asym_kernel(const double* __restrict__ M, int n, double* out) {
+  __shared__ double tile[32][33];
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+  if (bx > by) return;  // lower triangle of tiles suffices
+  double mx = 0.0;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int row = bx + r, col = by + threadIdx.x;
+    tile[r][threadIdx.x] = (row < n && col < n) ? M[(size_t)row * n + col] : 0.0;
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int row = by + r, col = bx + threadIdx.x;
+    if (row < n && col < n) { const double d = fabs(M[(size_t)row * n + col] - tile[threadIdx.x][r]); if (d > mx) mx = d; }
+  }
+  for (int o = 16; o > 0; o >>= 1) { const double t = __shfl_xor_sync(0xffffffffu, mx, o); if (t > mx) mx = t; }
+  if (threadIdx.x == 0 && mx > 0.0) atomic_max_nonneg(out, mx);
+}
+cudaError_t tdg_launch_asym(const double* M, int n, double* out, cudaStream_t s) {
+  dim3 block(32, 8), grid((n + 31) / 32, (n + 31) / 32);
+  asym_kernel<<<grid, block, 0, s>>>(M, n, out);
+  return cudaGetLastError();
+}
+
+__global__ void symsplit_kernel(const double* __restrict__ M, int n, double* __restrict__ S, double* __restrict__ N) {
+  __shared__ double tile[32][33];
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int row = bx + r, col = by + threadIdx.x;
+    tile[r][threadIdx.x] = (row < n && col < n) ? M[(size_t)row * n + col] : 0.0;   // M[bx+r][by+c]
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int row = by + r, col = bx + threadIdx.x;
+    if (row < n && col < n) {
+      const double a = M[(size_t)row * n + col], b = tile[threadIdx.x][r];       // M[row][col], M[col][row]
+      S[(size_t)row * n + col] = 0.5 * (a + b);
+      N[(size_t)row * n + col] = 0.5 * (a - b);
+    }
+  }
+}
+cudaError_t tdg_launch_symsplit(const double* M, int n, double* S, double* N, cudaStream_t s) {
+  dim3 block(32, 8), grid((n + 31) / 32, (n + 31) / 32);
+  symsplit_kernel<<<grid, block, 0, s>>>(M, n, S, N);
+  return cudaGetLastError();
+}
+
+__global__ void dmax_block_kernel(const double* const* __restrict__ mats, int nmat, int n, const DevShell* __restrict__ sh,
+                                  int ns, double* __restrict__ m) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= ns) return;
+  const DevShell si = sh[i], sj = sh[j];
+  const int ni = ncart(si.l), nj = ncart(sj.l);
+  double mx = 0.0;
+  for (int q = 0; q < nmat; ++q) {
+    const double* M = mats[q];
+    for (int a = 0; a < ni; ++a)
+      for (int b = 0; b < nj; ++b) {
+        const double v = fabs(M[(size_t)(si.bf_off + a) * n + sj.bf_off + b]);
+        if (v > mx) mx = v;
+      }
+  }
+  m[(size_t)i * ns + j] = mx;
+}
+__global__ void dmax_sym_kernel(int ns, double* __restrict__ m) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+  if (j >= ns || j >= i) return;
+  const double a = m[(size_t)i * ns + j], b = m[(size_t)j * ns + i];
+  const double v = a > b ? a : b;
+  m[(size_t)i * ns + j] = v;
+  m[(size_t)j * ns + i] = v;
+}
+cudaError_t tdg_launch_dmax(const double* const* mats_dev, int nmat, int n, const DevShell* sh, int ns, double* m, cudaStream_t s) {
+  dim3 block(128), grid((ns + 127) / 128, ns);
+  dmax_block_kernel<<<grid, block, 0, s>>>(mats_dev, nmat, n, sh, ns, m);
+  dmax_sym_kernel<<<grid, block, 0, s>>>(ns, m);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
+template <int N>
+__global__ void rys_test_kernel(int count, const double* __restrict__ T, const double* __restrict__ rho, double omega,
+                                const double* __restrict__ tab, double* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  double s2 = 1.0, ss = 1.0;
+  if (omega > 0.0) { s2 = omega * omega / (omega * omega + rho[i]); ss = sqrt(s2); }
+  double x[N], w[N];
+  rys_roots<N>(tab, s2 * T[i], x, w);
+  for (int r = 0; r < N; ++r) { out[(size_t)i * 2 * N + r] = x[r] * s2; out[(size_t)i * 2 * N + N + r] = w[r] * ss; }
+}
+cudaError_t tdg_launch_rys(int n, int count, const double* T, const double* rho, double omega, const double* tab, double* out, cudaStream_t s) {
+  const int nb = (count + 127) / 128;
+  switch (n) {
+    case 1: rys_test_kernel<1><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    case 2: rys_test_kernel<2><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    case 3: rys_test_kernel<3><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    case 4: rys_test_kernel<4><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    case 5: rys_test_kernel<5><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    case 6: rys_test_kernel<6><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    case 7: rys_test_kernel<7><<<nb, 128, 0, s>>>(count, T, rho, omega, tab, out); break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// FP64 FMA peak: 8 independent dependent-FMA chains per thread.
+__global__ void dfma_kernel(double* out, int iters, double a, double b) {
+  double v0 = threadIdx.x, v1 = v0 + 1, v2 = v0 + 2, v3 = v0 + 3, v4 = v0 + 4, v5 = v0 + 5, v6 = v0 + 6, v7 = v0 + 7;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      v0 = fma(v0, a, b); v1 = fma(v1, a, b); v2 = fma(v2, a, b); v3 = fma(v3, a, b);
+      v4 = fma(v4, a, b); v5 = fma(v5, a, b); v6 = fma(v6, a, b); v7 = fma(v7, a, b);
+    }
+  }
+  const double s = v0 + v1 + v2 + v3 + v4 + v5 + v6 + v7;
+  if (s == 123.456) out[0] = s;
+}
+cudaError_t tdg_run_fp64_peak(double ms, double* tflops) {
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  double* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, 8);
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int threads = 256, blocks = sms * 8;
+  int iters = 2000;
+  float t = 0.f;
+  double best = 0.0, spent = 0.0;
+  dfma_kernel<<<blocks, threads>>>(d, 100, 0.999999, 1e-7);  // warm-up
+  cudaDeviceSynchronize();
+  while (spent < ms) {
+    cudaEventRecord(e0);
+    dfma_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-7);
+    cudaEventRecord(e1);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    cudaEventElapsedTime(&t, e0, e1);
+    spent += t;
+    const double fl = 2.0 * 8 * 16 * (double)iters * threads * blocks;
+    const double tf = fl / (t * 1e-3) * 1e-12;
+    if (tf > best) best = tf;
+    if (t < 20.f) iters *= 2;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d);
+  *tflops = best;
+  return e != cudaSuccess ? e : cudaGetLastError();
+}

@@ -1,0 +1,121 @@
+// tdg_common.cuh — device data layout and small device helpers shared by the CUDA kernels of libtdgrad.
+// (Product code: shares nothing with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define TDG_WARP 32
+#define TDG_KW 32                 // kets per warp per work item
+#define TDG_WARPS 4               // warps per block
+#define TDG_KB (TDG_KW * TDG_WARPS)  // kets per block work item
+#define TDG_MAXP 8                // max canonical density pairs (J or K) per call
+
+// Shell-pair header (80 B).  The pair is oriented so that l(first) >= l(second) ("highest l first").
+struct __align__(16) PairHdr {
+  double A[3];    // centre of the first shell
+  double AB[3];   // A - B
+  double Q;       // Schwarz bound sqrt(max (mn|mn))
+  int32_t ish, jsh;      // INPUT shell indices of first/second shell
+  int32_t atomA, atomB;
+  int32_t offA, offB;    // first basis function of each shell
+};
+// Primitive-pair record: 8 doubles: p, Px, Py, Pz, Kab, a, b, (unused)
+#define TDG_PRIM_STRIDE 8
+
+struct DensPair { const double* X; const double* Y; double w; };
+
+struct KParams {
+  const PairHdr* bra_hdr; const double* bra_prim; int nbra; int nppb;
+  const PairHdr* ket_hdr; const double* ket_prim; int nket; int nppk;
+  const int* cum;        // [ntiles+1] cumulative number of block work items per bra tile
+  int ntiles; int same_bucket;
+  double tau; int density_weighted; const double* dmax; int nshell;
+  double CJ, CK;         // S9 weights of the density-weighted bound
+  uint32_t sample_mod, sample_seed;
+  int nJ; DensPair jp[TDG_MAXP];   // Gt_J = sum w (X_mn Y_ls + X_ls Y_mn)
+  int nK; DensPair kp[TDG_MAXP];   // Gt_K = sum w (X_ml Y_ns + X_nl Y_ms + X_ms Y_nl + X_ns Y_ml)
+  int nbf;
+  double cK, cLR, omega2; int use_lr;
+  double* grad;                    // [natom][3]
+  unsigned long long* counters;    // [3]: visited, computed, prim quartets
+  const double* rys_tab;
+};
+
+__host__ __device__ constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+
+// Cartesian exponent d (0:x 1:y 2:z) of component idx of shell l; order lx desc, then ly desc (reading S7).
+__host__ __device__ constexpr int cart_exp(int l, int idx, int d) {
+  int c = 0;
+  for (int lx = l; lx >= 0; --lx)
+    for (int ly = l - lx; ly >= 0; --ly) {
+      if (c == idx) return d == 0 ? lx : (d == 1 ? ly : l - lx - ly);
+      ++c;
+    }
+  return 0;
+}
+// packed runtime table: [l][idx] -> lx | ly<<4 | lz<<8
+__constant__ static uint16_t c_cart[4][10] = {
+  {0x000},
+  {0x001, 0x010, 0x100},
+  {0x002, 0x011, 0x101, 0x020, 0x110, 0x200},
+  {0x003, 0x012, 0x102, 0x021, 0x111, 0x201, 0x030, 0x120, 0x210, 0x300}};
+// per-component normalisation 1/sqrt((2lx-1)!!(2ly-1)!!(2lz-1)!!) (eq 38 "N"; O1)
+__host__ __device__ constexpr double dfact_odd(int n) { return n <= 0 ? 1.0 : (n == 1 ? 1.0 : (n == 2 ? 3.0 : 15.0)); }
+__constant__ static double c_cnorm[4][10] = {
+  {1.0},
+  {1.0, 1.0, 1.0},
+  {0.57735026918962576451, 1.0, 1.0, 0.57735026918962576451, 1.0, 0.57735026918962576451},
+  {0.25819888974716112568, 0.57735026918962576451, 0.57735026918962576451, 0.57735026918962576451, 1.0,
+   0.57735026918962576451, 0.25819888974716112568, 0.57735026918962576451, 0.57735026918962576451,
+   0.25819888974716112568}};
+
+// S12 subsample filter: fixed 64-bit finaliser on canonical INPUT shell-pair indices.
+__host__ __device__ inline uint64_t tdg_mix64(uint64_t z) {
+  z ^= z >> 30; z *= 0xbf58476d1ce4e5b9ULL;
+  z ^= z >> 27; z *= 0x94d049bb133111ebULL;
+  z ^= z >> 31;
+  return z;
+}
+__host__ __device__ inline bool tdg_sample_keep(int i, int j, int k, int l, uint32_t mod, uint32_t seed) {
+  if (mod == 0) return true;
+  if (i < j) { int t = i; i = j; j = t; }
+  if (k < l) { int t = k; k = l; l = t; }
+  uint64_t ij = (uint64_t)i * (uint64_t)(i + 1) / 2 + (uint64_t)j;
+  uint64_t kl = (uint64_t)k * (uint64_t)(k + 1) / 2 + (uint64_t)l;
+  uint64_t hi = ij > kl ? ij : kl, lo = ij > kl ? kl : ij;
+  uint64_t key = (hi << 32) ^ lo ^ ((uint64_t)seed * 0x9E3779B97F4A7C15ULL);
+  return (tdg_mix64(key) % mod) == 0;
+}
+
+// ---- Rys roots and weights (step a5) ----
+// Table layout (rys_tables.inc): for n: [interval][power, highest first][2n]; constants in __constant__.
+#include "rys_meta.inc"
+
+template <int N>
+__device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double T, double* __restrict__ x, double* __restrict__ w) {
+  if (T >= (double)rys_tmax(N)) {
+    double rT = 1.0 / T, rs = sqrt(rT);
+#pragma unroll
+    for (int r = 0; r < N; ++r) { x[r] = rys_inf(N, r) * rT; w[r] = rys_inf(N, N + r) * rs; }
+    return;
+  }
+  int i = (int)T;                       // RYS_H == 1
+  double u = (T - ((double)i + 0.5)) * 2.0;
+  const double* c = tab + rys_off(N) + i * ((RYS_DEG + 1) * 2 * N);
+  double v[2 * N];
+#pragma unroll
+  for (int f = 0; f < 2 * N; ++f) v[f] = __ldg(c + f);
+#pragma unroll
+  for (int k = 1; k <= RYS_DEG; ++k) {
+#pragma unroll
+    for (int f = 0; f < 2 * N; ++f) v[f] = fma(v[f], u, __ldg(c + k * 2 * N + f));
+  }
+#pragma unroll
+  for (int r = 0; r < N; ++r) { x[r] = v[r]; w[r] = v[N + r]; }
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}

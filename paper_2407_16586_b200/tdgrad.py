@@ -1,0 +1,169 @@
+"""ctypes binding of libtdgrad.so (include/tdgrad.h): argument marshalling only.
+
+Every step of the path runs inside the CUDA library; there is no CPU fallback: importing works without the
+library (so that workload generation can be used anywhere), but any call raises if ``libtdgrad.so`` is missing
+or no CUDA device is present.  Never imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtdgrad.so")
+NCLASS = 55
+_lib = None
+
+SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_plan", "tdg_schwarz", "tdg_gradient",
+           "tdg_energy", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
+
+
+class TdgError(RuntimeError):
+    pass
+
+
+class Options(C.Structure):
+    _fields_ = [("tau", C.c_double), ("density_weighted", C.c_int32), ("sample_mod", C.c_uint32), ("sample_seed", C.c_uint32)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("pairs_total", C.c_int64), ("pairs_kept", C.c_int64), ("quartets_visited", C.c_int64),
+                ("quartets_computed", C.c_int64), ("prim_quartets", C.c_int64), ("quartets_by_class", C.c_int64 * NCLASS),
+                ("ms_by_class", C.c_float * NCLASS), ("ms_prepare", C.c_float), ("ms_total", C.c_float), ("launches", C.c_int32)]
+
+    def asdict(self):
+        d = {k: getattr(self, k) for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets",
+                                           "ms_prepare", "ms_total", "launches")}
+        d["quartets_by_class"] = list(self.quartets_by_class)
+        d["ms_by_class"] = list(self.ms_by_class)
+        return d
+
+
+def lib():
+    """Load libtdgrad.so; raises (no fallback) when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise TdgError("libtdgrad.so not built: run `python -m paper_2407_16586_b200.build` (there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.tdg_strerror.restype = C.c_char_p
+        L.tdg_last_error.restype = C.c_char_p
+        L.tdg_last_error.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def class_name(cls: int) -> str:
+    pcs = [(la, lb) for la in range(4) for lb in range(la + 1)]
+    c1 = 0
+    while (c1 + 1) * (c1 + 2) // 2 <= cls:
+        c1 += 1
+    c2 = cls - c1 * (c1 + 1) // 2
+    s = "spdf"
+    return "(%s%s|%s%s)" % (s[pcs[c1][0]], s[pcs[c1][1]], s[pcs[c2][0]], s[pcs[c2][1]])
+
+
+def _ptr(x):
+    """Device/host address of a numpy array or a torch tensor."""
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return x.data_ptr()
+
+
+class Context:
+    """One tdg_ctx on one CUDA device."""
+
+    def __init__(self, device: int = 0):
+        self._h = C.c_void_p()
+        rc = lib().tdg_create(C.byref(self._h), C.c_int(device))
+        if rc != 0:
+            self._h = C.c_void_p()
+            raise TdgError("tdg_create(device=%d) failed: %s (no CPU fallback)" % (device, lib().tdg_strerror(rc).decode()))
+        self.natom = 0
+        self.nshell = 0
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise TdgError("%s: %s [%s]" % (what, lib().tdg_strerror(rc).decode(), lib().tdg_last_error(self._h).decode()))
+
+    def close(self):
+        if self._h:
+            lib().tdg_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_system(self, sysm):
+        xyz = np.ascontiguousarray(sysm.xyz, dtype=np.float64)
+        sh = np.ascontiguousarray(sysm.shells, dtype=np.int32)
+        ex = np.ascontiguousarray(sysm.exps, dtype=np.float64)
+        co = np.ascontiguousarray(sysm.coefs, dtype=np.float64)
+        rc = lib().tdg_set_system(self._h, C.c_int(xyz.shape[0]), C.c_void_p(xyz.ctypes.data), C.c_int(sh.shape[0]),
+                                  C.c_void_p(sh.ctypes.data), C.c_int(ex.shape[0]), C.c_void_p(ex.ctypes.data), C.c_void_p(co.ctypes.data))
+        self._check(rc, "tdg_set_system")
+        self.natom, self.nshell = int(xyz.shape[0]), int(sh.shape[0])
+
+    def nbf(self) -> int:
+        n = C.c_int()
+        self._check(lib().tdg_nbf(self._h, C.byref(n)), "tdg_nbf")
+        return n.value
+
+    def plan(self, tau=0.0, density_weighted=0, sample_mod=0, sample_seed=0):
+        opt = Options(tau, density_weighted, sample_mod, sample_seed)
+        self._check(lib().tdg_plan(self._h, C.byref(opt)), "tdg_plan")
+
+    def schwarz(self) -> np.ndarray:
+        out = np.zeros((self.nshell, self.nshell))
+        self._check(lib().tdg_schwarz(self._h, C.c_void_p(out.ctypes.data)), "tdg_schwarz")
+        return out
+
+    def gradient(self, pairs, wJ, wK, cJ, cK, cLR, omega, stream=None, out=None, want_stats=True):
+        """pairs: list of (A, B), all numpy arrays (host) or all CUDA torch tensors (device), nbf x nbf float64 row-major.
+        Returns (grad [natom,3] numpy or the given ``out`` tensor, stats dict or None)."""
+        npair = len(pairs)
+        on_dev = 0 if isinstance(pairs[0][0], np.ndarray) else 1
+        keep = []
+        if not on_dev:
+            for a, b in pairs:
+                keep.append((np.ascontiguousarray(a, dtype=np.float64), np.ascontiguousarray(b, dtype=np.float64)))
+        else:
+            for a, b in pairs:
+                assert a.is_cuda and b.is_cuda and a.is_contiguous() and b.is_contiguous()
+                keep.append((a, b))
+        PA = (C.c_void_p * npair)(*[_ptr(a) for a, _ in keep])
+        PB = (C.c_void_p * npair)(*[_ptr(b) for _, b in keep])
+        wJ = np.ascontiguousarray(wJ, dtype=np.float64)
+        wK = np.ascontiguousarray(wK, dtype=np.float64)
+        st = Stats() if want_stats else None
+        if out is None:
+            g = np.zeros((self.natom, 3))
+            gptr, g_dev = g.ctypes.data, 0
+        else:
+            g = out
+            gptr, g_dev = out.data_ptr(), 1
+        rc = lib().tdg_gradient(self._h, C.c_int(npair), PA, PB, C.c_int(on_dev), C.c_void_p(wJ.ctypes.data), C.c_void_p(wK.ctypes.data),
+                                C.c_double(cJ), C.c_double(cK), C.c_double(cLR), C.c_double(omega),
+                                C.c_void_p(stream if stream else 0), C.c_void_p(gptr), C.c_int(g_dev),
+                                C.byref(st) if st is not None else None)
+        self._check(rc, "tdg_gradient")
+        return g, (st.asdict() if st is not None else None)
+
+    def rys(self, n, T, rho=None, omega=0.0) -> np.ndarray:
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        rho = np.ones_like(T) if rho is None else np.ascontiguousarray(rho, dtype=np.float64)
+        out = np.zeros((T.shape[0], 2 * n))
+        rc = lib().tdg_rys(self._h, C.c_int(n), C.c_int(T.shape[0]), C.c_void_p(T.ctypes.data), C.c_void_p(rho.ctypes.data),
+                           C.c_double(omega), C.c_void_p(out.ctypes.data))
+        self._check(rc, "tdg_rys")
+        return out
+
+    def fp64_peak(self, ms=300.0) -> float:
+        v = C.c_double()
+        self._check(lib().tdg_fp64_peak(self._h, C.c_double(ms), C.byref(v)), "tdg_fp64_peak")
+        return v.value

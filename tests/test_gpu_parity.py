@@ -1,0 +1,165 @@
+"""GPU parity tests: libtdgrad (through the C ABI binding) against the CPU oracle, element by element.
+
+Tolerance (BASELINE.json north_star; reading S13): max|dg| <= 1e-9 E_h/bohr and max|dg|/max|g| <= 1e-10.
+Integer results (pair / quartet counts) must be identical.
+"""
+import numpy as np
+import pytest
+
+from paper_2407_16586_b200 import workload as wl
+from tests.helpers import CALL, densities, tiny_system
+
+pytestmark = pytest.mark.gpu
+
+ABS_TOL = 1e-9
+REL_TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2407_16586_b200 import tdgrad
+
+    c = tdgrad.Context(0)
+    yield c
+    c.close()
+
+
+def _compare(g, ref):
+    d = np.max(np.abs(g - ref))
+    assert d <= ABS_TOL, d
+    assert d / np.max(np.abs(ref)) <= REL_TOL, d / np.max(np.abs(ref))
+
+
+def _run_both(ctx, orc, s, pairs, wJ, wK, call=CALL, sample_mod=0, sample_seed=0, tau=None, dw=None):
+    tau = s.tau if tau is None else tau
+    dw = s.density_weighted if dw is None else dw
+    ctx.set_system(s)
+    ctx.plan(tau, dw, sample_mod, sample_seed)
+    g, st = ctx.gradient(pairs, wJ, wK, call["cJ"], call["cK"], call["cLR"], call["omega"])
+    ref, rst = orc.gradient(s, pairs, wJ, wK, call["cJ"], call["cK"], call["cLR"], call["omega"], tau=tau, density_weighted=dw,
+                            sample_mod=sample_mod, sample_seed=sample_seed)
+    return g, st, ref, rst
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("omega", [0.0, 0.3, 5.0])
+def test_rys_moments_vs_oracle_boys(ctx, orc, n, omega):
+    """sum_r w_r x_r^k == G_k(T, rho, omega), k < 2n, with G the oracle's (attenuated) Boys vector (O2/O3, S8)."""
+    rng = np.random.default_rng(n)
+    T = np.concatenate([[0.0, 1e-7, 0.3, 1.0, 39.999, 40.0, 77.9, 78.0, 150.0, 3e4], rng.uniform(0, 90, 200), 10 ** rng.uniform(-6, 5, 50)])
+    rho = rng.uniform(0.05, 50.0, T.shape[0])
+    out = ctx.rys(n, T, rho, omega)
+    for i in range(T.shape[0]):
+        x, w = out[i, :n], out[i, n:]
+        G = orc.boys_op(2 * n - 1, T[i], rho[i], omega) if omega > 0 else orc.boys(2 * n - 1, T[i])
+        for k in range(2 * n):
+            assert abs(np.sum(w * x ** k) - G[k]) <= 3e-13 * G[k], (n, omega, T[i], k)
+
+
+@pytest.mark.parametrize("with_f", [False, True])
+def test_schwarz_vs_oracle(ctx, orc, with_f):
+    s = tiny_system(with_f=with_f)
+    ctx.set_system(s)
+    Q = ctx.schwarz()
+    ref = orc.schwarz(s)
+    assert np.max(np.abs(Q - ref) / ref) < 1e-12
+
+
+def test_schwarz_cfg1(ctx, orc):
+    s = wl.make_system(1)
+    ctx.set_system(s)
+    Q = ctx.schwarz()
+    ref = orc.schwarz(s)
+    big = ref > 1e-20
+    assert np.max(np.abs(Q[big] - ref[big]) / ref[big]) < 1e-10
+    assert np.max(np.abs(Q[~big] - ref[~big])) < 1e-20
+
+
+@pytest.mark.parametrize("with_f", [False, True])
+def test_tiny_system_all_classes(ctx, orc, with_f):
+    s = tiny_system(with_f=with_f)
+    D, P, T = densities(s.nbf)
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK)
+    _compare(g, ref)
+    for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets"):
+        assert st[k] == rst[k], k
+
+
+def test_tiny_general_pairs_and_weights(ctx, orc):
+    """Arbitrary nonsymmetric A != B pairs and weights exercise the sym/antisym split of the K term."""
+    s = tiny_system(with_f=False)
+    rng = np.random.default_rng(5)
+    n = s.nbf
+    M = [rng.standard_normal((n, n)) for _ in range(4)]
+    pairs = [(M[0], M[1]), (M[2], M[2]), (M[3], M[0] + M[0].T)]
+    wJ, wK = np.array([0.7, -1.3, 0.4]), np.array([1.1, 0.5, -0.8])
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK)
+    _compare(g, ref)
+
+
+def test_tiny_no_lr_and_no_exchange(ctx, orc):
+    s = tiny_system(with_f=False)
+    D, P, T = densities(s.nbf)
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    for call in (dict(cJ=1.0, cK=0.3, cLR=0.0, omega=0.0), dict(cJ=1.0, cK=0.0, cLR=0.0, omega=0.3), dict(cJ=0.0, cK=0.0, cLR=1.0, omega=0.7)):
+        g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, call=call)
+        _compare(g, ref)
+
+
+def test_cfg0_golden_and_oracle(ctx, orc):
+    import os
+
+    s = wl.make_system(0)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(0))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK)
+    _compare(g, ref)
+    assert st["quartets_computed"] == rst["quartets_computed"] == 3081
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "cfg0_gradient.txt"))
+    _compare(g, gold)
+    assert np.max(np.abs(g.sum(axis=0))) < 1e-10
+
+
+def test_cfg1_full(ctx, orc):
+    s = wl.make_system(1)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK)
+    _compare(g, ref)
+    for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets"):
+        assert st[k] == rst[k], (k, st[k], rst[k])
+
+
+def test_cfg1_density_weighted_screening(ctx, orc):
+    s = wl.make_system(1)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, tau=1e-9, dw=1)
+    _compare(g, ref)
+    assert st["quartets_visited"] == rst["quartets_visited"]
+    assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 5
+    assert st["quartets_computed"] < st["quartets_visited"]
+
+
+def test_cfg2_f_shells_subsample(ctx, orc):
+    s = wl.make_system(2)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(2))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, sample_mod=1500, sample_seed=11)
+    _compare(g, ref)
+    assert st["pairs_kept"] == rst["pairs_kept"]
+    assert st["quartets_visited"] == rst["quartets_visited"]
+    assert st["quartets_computed"] == rst["quartets_computed"]
+
+
+@pytest.mark.slow
+def test_cfg3_subsample_bench_configuration(ctx, orc):
+    """256 waters, the launch configuration bench.py times, on a deterministic subsample both sides evaluate (S12)."""
+    s = wl.make_system(3)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(3))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, sample_mod=40000, sample_seed=3)
+    _compare(g, ref)
+    assert st["pairs_kept"] == rst["pairs_kept"]
+    assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 3

@@ -1,4 +1,4 @@
-"""Host-side check of the generated Rys tables (paper_2407_16586_b200/csrc/rys_tables.inc).
+"""Host-side check of the generated Rys tables (paper_2407_16586_b200/csrc/rys_meta.inc, rys_tables.inc).
 
 Pin (independent of the generator's Golub-Welsch arithmetic): an n-point Gauss rule for the weight
 exp(-T x)/(2 sqrt x) on [0,1] must reproduce the moments F_k(T), k = 0..2n-1 (Rys
@@ -12,24 +12,21 @@ import numpy as np
 import pytest
 from scipy import special
 
-INC = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2407_16586_b200", "csrc", "rys_tables.inc")
+CSRC = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2407_16586_b200", "csrc")
 
 
 def _load():
-    txt = open(INC).read()
-    deg = int(re.search(r"#define RYS_DEG (\d+)", txt).group(1))
-    h = float(re.search(r"#define RYS_H (\S+)", txt).group(1))
-    nmax = int(re.search(r"#define RYS_NMAX (\d+)", txt).group(1))
-
-    def arr(name):
-        body = re.search(name + r"[^=]*=\s*\{(.*?)\};", txt, re.S).group(1)
-        return np.array([float(x) for x in re.findall(r"[-+]?\d\.?\d*(?:[eE][-+]?\d+)?", body)])
-
-    tmax = arr("RYS_TMAX").astype(int)
-    off = arr("RYS_OFF").astype(int)
-    body = re.search(r"RYS_INF[^=]*=\s*\{(.*?)\};", txt, re.S).group(1)
-    inf = [np.array([float(x) for x in row.split(",") if x.strip()]) for row in re.findall(r"\{([^{}]*)\}", body)]
-    tab = arr("RYS_TAB")
+    meta = open(os.path.join(CSRC, "rys_meta.inc")).read()
+    txt = open(os.path.join(CSRC, "rys_tables.inc")).read()
+    deg = int(re.search(r"#define RYS_DEG (\d+)", meta).group(1))
+    h = float(re.search(r"#define RYS_H (\S+)", meta).group(1))
+    nmax = int(re.search(r"#define RYS_NMAX (\d+)", meta).group(1))
+    num = r"[-+]?\d+\.?\d*(?:[eE][-+]?\d+)?"
+    tmax = np.array([int(x) for x in re.findall(r"\d+", re.search(r"rys_tmax.*?=\s*\{(.*?)\}", meta).group(1))])
+    off = np.array([int(x) for x in re.findall(r"\d+", re.search(r"rys_off.*?=\s*\{(.*?)\}", meta).group(1))])
+    body = meta[meta.index("rys_inf(int n, int r)"):]
+    inf = [np.array([float(x) for x in re.findall(num, row)]) for row in re.findall(r"\{([^{}]*)\},", body)]
+    tab = np.array([float(x) for x in re.findall(num, txt[txt.index("= {"):])])
     return deg, h, nmax, tmax, off, inf, tab
 
 
