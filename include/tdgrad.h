@@ -63,6 +63,7 @@ typedef struct {
   int64_t quartets_computed;           /* ... and the density-weighted test and the subsample filter      */
   int64_t prim_quartets;               /* primitive quartets of the computed ones                         */
   int64_t quartets_by_class[TDG_NCLASS];
+  int64_t prim_quartets_by_class[TDG_NCLASS];
   float ms_by_class[TDG_NCLASS];       /* CUDA-event time of each class (only when stats != NULL)         */
   float ms_prepare;                    /* density preparation (a3)                                        */
   float ms_total;                      /* whole tdg_gradient device time                                  */

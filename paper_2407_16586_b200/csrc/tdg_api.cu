@@ -451,6 +451,7 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
       stats->quartets_visited += (int64_t)cnt[3 * w]; stats->quartets_computed += (int64_t)cnt[3 * w + 1];
       stats->prim_quartets += (int64_t)cnt[3 * w + 2];
       stats->quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 1];
+      stats->prim_quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 2];
       float ms = 0.f;
       cudaEventElapsedTime(&ms, evs[w], w + 1 < evs.size() ? evs[w + 1] : ev2);
       stats->ms_by_class[ctx->work[w].cls] += ms;

@@ -31,12 +31,14 @@ class Options(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("pairs_total", C.c_int64), ("pairs_kept", C.c_int64), ("quartets_visited", C.c_int64),
                 ("quartets_computed", C.c_int64), ("prim_quartets", C.c_int64), ("quartets_by_class", C.c_int64 * NCLASS),
+                ("prim_quartets_by_class", C.c_int64 * NCLASS),
                 ("ms_by_class", C.c_float * NCLASS), ("ms_prepare", C.c_float), ("ms_total", C.c_float), ("launches", C.c_int32)]
 
     def asdict(self):
         d = {k: getattr(self, k) for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets",
                                            "ms_prepare", "ms_total", "launches")}
         d["quartets_by_class"] = list(self.quartets_by_class)
+        d["prim_quartets_by_class"] = list(self.prim_quartets_by_class)
         d["ms_by_class"] = list(self.ms_by_class)
         return d
 
@@ -55,14 +57,34 @@ def lib():
     return _lib
 
 
-def class_name(cls: int) -> str:
+def class_ls(cls: int):
+    """(la, lb, lc, ld) of quartet class index cls = c1 (c1+1)/2 + c2 over pair classes c = la (la+1)/2 + lb."""
     pcs = [(la, lb) for la in range(4) for lb in range(la + 1)]
     c1 = 0
     while (c1 + 1) * (c1 + 2) // 2 <= cls:
         c1 += 1
     c2 = cls - c1 * (c1 + 1) // 2
+    return pcs[c1] + pcs[c2]
+
+
+def class_name(cls: int) -> str:
     s = "spdf"
-    return "(%s%s|%s%s)" % (s[pcs[c1][0]], s[pcs[c1][1]], s[pcs[c2][0]], s[pcs[c2][1]])
+    la, lb, lc, ld = class_ls(cls)
+    return "(%s%s|%s%s)" % (s[la], s[lb], s[lc], s[ld])
+
+
+def model_flops(cls: int, quartets: int, prim_quartets: int) -> float:
+    """Algorithmic FP64 FLOPs of `quartets` contracted / `prim_quartets` primitive quartets of class `cls`
+    (Rys-direct model of SURVEY.md 8(d) / DESIGN.md "Work per unit"; two operators)."""
+    la, lb, lc, ld = class_ls(cls)
+    L = la + lb + lc + ld
+    nr = (L + 1) // 2 + 1
+    nc = 1
+    for l in (la, lb, lc, ld):
+        nc *= (l + 1) * (l + 2) // 2
+    c2d = 3 * (6 * (la + lb + 2) * (lc + ld + 2) + 2 * (la + 1) * (lb + 2) * (lc + 2) * (ld + 2)) + 27 * (la + 1) * (lb + 1) * (lc + 1) * (ld + 1)
+    per_prim = 2 * nr * c2d + nc * nr * 90 + 2 * (60 + 20 * nr)
+    return float(prim_quartets) * per_prim + float(quartets) * nc * 100
 
 
 def _ptr(x):
