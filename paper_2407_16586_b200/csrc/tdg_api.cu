@@ -70,6 +70,7 @@ struct tdg_ctx {
   std::vector<DevShell> shells;
   double *d_xyz = nullptr, *d_exps = nullptr, *d_cn = nullptr, *d_Q = nullptr, *d_rys = nullptr;
   DevShell* d_shells = nullptr;
+  int* d_bf2sh = nullptr;
   bool have_Q = false;
   // plan
   bool planned = false;
@@ -105,7 +106,7 @@ static void free_plan(tdg_ctx* c) {
 static void free_system(tdg_ctx* c) {
   free_plan(c);
   cudaFree(c->d_xyz); cudaFree(c->d_exps); cudaFree(c->d_cn); cudaFree(c->d_Q); cudaFree(c->d_shells);
-  cudaFree(c->d_grad); cudaFree(c->d_dmax);
+  cudaFree(c->d_grad); cudaFree(c->d_dmax); cudaFree(c->d_bf2sh); c->d_bf2sh = nullptr;
   c->d_xyz = c->d_exps = c->d_cn = c->d_Q = c->d_grad = c->d_dmax = nullptr; c->d_shells = nullptr;
   for (auto& s : c->scratch) cudaFree(s.second);
   c->scratch.clear(); c->scratch_used.clear();
@@ -193,6 +194,13 @@ extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int ns
     off += ncart(sh.l);
   }
   ctx->nbf = off;
+  {
+    std::vector<int> bf2sh(off);
+    for (int sidx = 0; sidx < nshell; ++sidx)
+      for (int f = 0; f < ncart(ctx->shells[sidx].l); ++f) bf2sh[ctx->shells[sidx].bf_off + f] = sidx;
+    CK(cudaMalloc(&ctx->d_bf2sh, sizeof(int) * off));
+    CK(cudaMemcpy(ctx->d_bf2sh, bf2sh.data(), sizeof(int) * off, cudaMemcpyHostToDevice));
+  }
   CK(cudaMalloc(&ctx->d_xyz, sizeof(double) * 3 * natom));
   CK(cudaMalloc(&ctx->d_exps, sizeof(double) * nprim_total));
   CK(cudaMalloc(&ctx->d_cn, sizeof(double) * nprim_total));
@@ -341,7 +349,7 @@ static void* scratch_get(tdg_ctx* ctx, size_t bytes) {
 }
 
 namespace {
-struct Canon { const double* S; const double* N; };   // symmetric / antisymmetric parts (N == nullptr: symmetric input)
+struct Group { std::vector<int> pairs; std::vector<int> canon; };   // canonical matrix id = 2*unique + (0: sym part, 1: antisym part)
 }
 
 static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int on_dev,
@@ -353,112 +361,134 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
   if (stats) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventCreate(&ev2); cudaEventRecord(ev0, st); }
   // unique input matrices -> device pointers
-  std::map<const double*, const double*> dev;   // input pointer -> device pointer
+  std::vector<const double*> uniq, udev;
+  auto uid = [&](const double* M) { for (size_t i = 0; i < uniq.size(); ++i) if (uniq[i] == M) return (int)i; return -1; };
   for (int k = 0; k < npair; ++k)
     for (const double* M : {A[k], B[k]}) {
-      if (dev.count(M)) continue;
-      if (on_dev) dev[M] = M;
-      else {
-        double* d = (double*)scratch_get(ctx, mbytes);
-        if (!d) { ctx->err = "device allocation of a density matrix failed"; return TDG_ENOMEM; }
-        CK(cudaMemcpyAsync(d, M, mbytes, cudaMemcpyHostToDevice, st));
-        dev[M] = d;
+      if (uid(M) >= 0) continue;
+      const double* d = M;
+      if (!on_dev) {
+        double* buf = (double*)scratch_get(ctx, mbytes);
+        if (!buf) { ctx->err = "device allocation of a density matrix failed"; return TDG_ENOMEM; }
+        CK(cudaMemcpyAsync(buf, M, mbytes, cudaMemcpyHostToDevice, st));
+        d = buf;
       }
+      uniq.push_back(M); udev.push_back(d);
     }
-  // symmetric / antisymmetric split (K(A,B) = K(As,Bs) + K(An,Bn) after 8-fold symmetrisation)
-  std::map<const double*, Canon> canon;
+  if (uniq.size() > 16) return TDG_EINVAL;
+  // which inputs are nonsymmetric (their antisymmetric part takes a slot; reading R1 of DESIGN.md)
+  double as[16];
   {
     double* d_as = (double*)scratch_get(ctx, 256);
     if (!d_as) return TDG_ENOMEM;
-    std::vector<const double*> keys;
-    for (auto& kv : dev) keys.push_back(kv.first);
-    if (keys.size() > 32) return TDG_EINVAL;
     CK(cudaMemsetAsync(d_as, 0, 256, st));
-    for (size_t i = 0; i < keys.size(); ++i) CK(tdg_launch_asym(dev[keys[i]], n, d_as + i, st));
-    double as[32];
-    CK(cudaMemcpyAsync(as, d_as, sizeof(double) * keys.size(), cudaMemcpyDeviceToHost, st));
+    for (size_t i = 0; i < uniq.size(); ++i) CK(tdg_launch_asym(udev[i], n, d_as + i, st));
+    CK(cudaMemcpyAsync(as, d_as, sizeof(double) * uniq.size(), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    for (size_t i = 0; i < keys.size(); ++i) {
-      if (as[i] == 0.0) canon[keys[i]] = Canon{dev[keys[i]], nullptr};
-      else {
-        double* S = (double*)scratch_get(ctx, mbytes); double* N = (double*)scratch_get(ctx, mbytes);
-        if (!S || !N) { ctx->err = "device allocation of symmetrised densities failed"; return TDG_ENOMEM; }
-        CK(tdg_launch_symsplit(dev[keys[i]], n, S, N, st));
-        canon[keys[i]] = Canon{S, N};
-      }
-    }
   }
-  KParams P{};
-  P.nJ = 0; P.nK = 0;
+  const bool useK = (cK != 0.0 || cLR != 0.0);
+  // groups of density pairs whose canonical matrices fit the 4 slots of the packed array
+  std::vector<Group> groups;
   double CJ = 0.0, CKs = 0.0;
   for (int k = 0; k < npair; ++k) {
-    const Canon& a = canon[A[k]]; const Canon& b = canon[B[k]];
     CJ += std::fabs(wJ[k] * cJ); CKs += std::fabs(wK[k]);
-    if (wJ[k] * cJ != 0.0) {
-      if (P.nJ >= TDG_MAXP) return TDG_EINVAL;
-      P.jp[P.nJ++] = DensPair{a.S, b.S, 4.0 * wJ[k] * cJ};
-    }
-    if (wK[k] != 0.0 && (cK != 0.0 || cLR != 0.0)) {
-      if (P.nK + 2 > TDG_MAXP) return TDG_EINVAL;
-      P.kp[P.nK++] = DensPair{a.S, b.S, -2.0 * wK[k]};
-      if (a.N && b.N) P.kp[P.nK++] = DensPair{a.N, b.N, -2.0 * wK[k]};
-    }
+    const bool doJ = wJ[k] * cJ != 0.0, doK = wK[k] != 0.0 && useK;
+    if (!doJ && !doK) continue;
+    const int ua = uid(A[k]), ub = uid(B[k]);
+    std::vector<int> need = {2 * ua, 2 * ub};
+    if (doK && as[ua] != 0.0 && as[ub] != 0.0) { need.push_back(2 * ua + 1); need.push_back(2 * ub + 1); }
+    auto merged = [&](const std::vector<int>& base) {
+      std::vector<int> r = base;
+      for (int c : need) if (std::find(r.begin(), r.end(), c) == r.end()) r.push_back(c);
+      return r;
+    };
+    if (groups.empty() || merged(groups.back().canon).size() > 4) groups.push_back(Group{});
+    groups.back().canon = merged(groups.back().canon);
+    groups.back().pairs.push_back(k);
   }
   CKs *= std::fabs(cK) + std::fabs(cLR);
+  KParams P{};
   P.CJ = CJ; P.CK = CKs;
   P.tau = ctx->opt.tau; P.density_weighted = (ctx->opt.tau > 0.0) ? ctx->opt.density_weighted : 0;
   P.nshell = ctx->nshell; P.sample_mod = ctx->opt.sample_mod; P.sample_seed = ctx->opt.sample_seed;
   P.nbf = n; P.cK = cK; P.cLR = cLR; P.omega2 = omega * omega; P.use_lr = (cLR != 0.0) ? 1 : 0;
   P.grad = ctx->d_grad; P.rys_tab = ctx->d_rys;
+  int aux_launches = (int)uniq.size();
   if (P.density_weighted) {   // d_ij over ALL input matrices (reading S9)
     if (!ctx->d_dmax) CK(cudaMalloc(&ctx->d_dmax, sizeof(double) * (size_t)ctx->nshell * ctx->nshell));
-    std::vector<const double*> mats;
-    for (auto& kv : dev) mats.push_back(kv.second);
     const double** d_list = (const double**)scratch_get(ctx, 512);
     if (!d_list) return TDG_ENOMEM;
-    CK(cudaMemcpyAsync(d_list, mats.data(), sizeof(double*) * mats.size(), cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));   // mats is a local vector
-    CK(tdg_launch_dmax(d_list, (int)mats.size(), n, ctx->d_shells, ctx->nshell, ctx->d_dmax, st));
+    CK(cudaMemcpyAsync(d_list, udev.data(), sizeof(double*) * udev.size(), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    CK(tdg_launch_dmax(d_list, (int)udev.size(), n, ctx->d_shells, ctx->nshell, ctx->d_dmax, st));
     P.dmax = ctx->d_dmax;
+    aux_launches += 2;
   }
+  double* pk = (double*)scratch_get(ctx, 4 * mbytes);
+  if (!pk) { ctx->err = "device allocation of the packed density array failed"; return TDG_ENOMEM; }
+  P.pk = pk;
+  const size_t nw = ctx->work.size();
   CK(cudaMemsetAsync(ctx->d_grad, 0, sizeof(double) * 3 * ctx->natom, st));
-  CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * (ctx->work.size() * 3 + 3), st));
+  CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * (nw * 3 + 3), st));
   if (stats) cudaEventRecord(ev1, st);
   int launches = 0;
   std::vector<cudaEvent_t> evs;
-  for (size_t w = 0; w < ctx->work.size(); ++w) {
-    const Work& W = ctx->work[w];
-    const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
-    tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb);
-    if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
-    P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
-    P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
-    P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
-    P.counters = ctx->d_counters + 3 * w;
-    if (stats) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); evs.push_back(e); }
-    fn(P, W.nblocks, st);
-    ++launches;
+  std::vector<int> ev_cls;
+  for (size_t gi = 0; gi < groups.size(); ++gi) {
+    const Group& G = groups[gi];
+    PackSrc ps{};
+    for (size_t m = 0; m < G.canon.size(); ++m) { ps.src[m] = udev[G.canon[m] / 2]; ps.kind[m] = G.canon[m] & 1; }
+    CK(tdg_launch_pack(ps, n, ctx->d_bf2sh, ctx->d_shells, pk, st));
+    ++aux_launches;
+    auto slot = [&](int c) { return (int)(std::find(G.canon.begin(), G.canon.end(), c) - G.canon.begin()); };
+    for (int t = 0; t < 16; ++t) { P.MJ[t] = 0.0; P.MK[t] = 0.0; }
+    for (int k : G.pairs) {
+      const int ua = uid(A[k]), ub = uid(B[k]);
+      const int sa = slot(2 * ua), sb = slot(2 * ub);
+      const double wj = 4.0 * wJ[k] * cJ, wk = useK ? -2.0 * wK[k] : 0.0;
+      P.MJ[4 * sa + sb] += wj; P.MJ[4 * sb + sa] += wj;
+      P.MK[4 * sa + sb] += wk; P.MK[4 * sb + sa] += wk;
+      if (wk != 0.0 && as[ua] != 0.0 && as[ub] != 0.0) {
+        const int na = slot(2 * ua + 1), nb = slot(2 * ub + 1);
+        P.MK[4 * na + nb] += wk; P.MK[4 * nb + na] += wk;
+      }
+    }
+    for (size_t w = 0; w < nw; ++w) {
+      const Work& W = ctx->work[w];
+      const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
+      tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb);
+      if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+      P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
+      P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
+      P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
+      P.counters = ctx->d_counters + 3 * (gi == 0 ? w : nw);   // quartet counts come from the first group only
+      if (stats) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); evs.push_back(e); ev_cls.push_back(W.cls); }
+      fn(P, W.nblocks, st);
+      ++launches;
+    }
   }
   CK(cudaGetLastError());
   if (stats) {
     cudaEventRecord(ev2, st);
     CK(cudaStreamSynchronize(st));
-    std::vector<unsigned long long> cnt(ctx->work.size() * 3 + 3);
+    std::vector<unsigned long long> cnt(nw * 3 + 3);
     CK(cudaMemcpy(cnt.data(), ctx->d_counters, sizeof(unsigned long long) * cnt.size(), cudaMemcpyDeviceToHost));
     std::memset(stats, 0, sizeof(*stats));
     stats->pairs_total = ctx->pairs_total; stats->pairs_kept = ctx->pairs_kept;
-    for (size_t w = 0; w < ctx->work.size(); ++w) {
+    for (size_t w = 0; w < nw; ++w) {
       stats->quartets_visited += (int64_t)cnt[3 * w]; stats->quartets_computed += (int64_t)cnt[3 * w + 1];
       stats->prim_quartets += (int64_t)cnt[3 * w + 2];
       stats->quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 1];
       stats->prim_quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 2];
+    }
+    for (size_t e = 0; e < evs.size(); ++e) {
       float ms = 0.f;
-      cudaEventElapsedTime(&ms, evs[w], w + 1 < evs.size() ? evs[w + 1] : ev2);
-      stats->ms_by_class[ctx->work[w].cls] += ms;
+      cudaEventElapsedTime(&ms, evs[e], e + 1 < evs.size() ? evs[e + 1] : ev2);
+      stats->ms_by_class[ev_cls[e]] += ms;
     }
     cudaEventElapsedTime(&stats->ms_prepare, ev0, ev1);
     cudaEventElapsedTime(&stats->ms_total, ev0, ev2);
-    stats->launches = launches + (int)dev.size() + (P.density_weighted ? 2 : 0);
+    stats->launches = launches + aux_launches;
     for (auto e : evs) cudaEventDestroy(e);
     cudaEventDestroy(ev0); cudaEventDestroy(ev1); cudaEventDestroy(ev2);
   }

@@ -192,6 +192,31 @@ cudaError_t tdg_launch_symsplit(const double* M, int n, double* S, double* N, cu
   return cudaGetLastError();
 }
 
+__global__ void pack_kernel(const PackSrc ps, int n, const int* __restrict__ bf2sh, const DevShell* __restrict__ sh,
+                            double* __restrict__ pk) {
+  const int col = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
+  if (col >= n) return;
+  const DevShell sI = sh[bf2sh[row]], sK = sh[bf2sh[col]];
+  const int nI = ncart(sI.l), nK = ncart(sK.l), a = row - sI.bf_off, c = col - sK.bf_off;
+  double v[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    v[m] = 0.0;
+    if (ps.src[m]) {
+      const double x = ps.src[m][(size_t)row * n + col], y = ps.src[m][(size_t)col * n + row];
+      v[m] = ps.kind[m] == 0 ? 0.5 * (x + y) : 0.5 * (x - y);
+    }
+  }
+  double* dst = pk + 4 * ((size_t)sI.bf_off * n + (size_t)nI * sK.bf_off) + (size_t)(a * nK + c) * 4;
+  reinterpret_cast<double2*>(dst)[0] = make_double2(v[0], v[1]);
+  reinterpret_cast<double2*>(dst)[1] = make_double2(v[2], v[3]);
+}
+cudaError_t tdg_launch_pack(const PackSrc& ps, int n, const int* bf2sh, const DevShell* sh, double* pk, cudaStream_t s) {
+  dim3 block(128), grid((n + 127) / 128, n);
+  pack_kernel<<<grid, block, 0, s>>>(ps, n, bf2sh, sh, pk);
+  return cudaGetLastError();
+}
+
 __global__ void dmax_block_kernel(const double* const* __restrict__ mats, int nmat, int n, const DevShell* __restrict__ sh,
                                   int ns, double* __restrict__ m) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;

@@ -22,7 +22,6 @@ struct __align__(16) PairHdr {
 // Primitive-pair record: 8 doubles: p, Px, Py, Pz, Kab, a, b, (unused)
 #define TDG_PRIM_STRIDE 8
 
-struct DensPair { const double* X; const double* Y; double w; };
 
 struct KParams {
   const PairHdr* bra_hdr; const double* bra_prim; int nbra; int nppb;
@@ -32,8 +31,10 @@ struct KParams {
   double tau; int density_weighted; const double* dmax; int nshell;
   double CJ, CK;         // S9 weights of the density-weighted bound
   uint32_t sample_mod, sample_seed;
-  int nJ; DensPair jp[TDG_MAXP];   // Gt_J = sum w (X_mn Y_ls + X_ls Y_mn)
-  int nK; DensPair kp[TDG_MAXP];   // Gt_K = sum w (X_ml Y_ns + X_nl Y_ms + X_ms Y_nl + X_ns Y_ml)
+  // Packed densities (tdg_internal.h): 4 canonical matrices interleaved, shell-blocked.  With u = pk(ik)[a,c][.],
+  // v = pk(jl)[b,d][.], s = pk(jk)[b,c][.], t = pk(il)[a,d][.]:  Gt_K = u.MK.v + s.MK.t ;  Gt_J = pk(ij)[a,b].MJ.pk(kl)[c,d]
+  // (MJ, MK symmetric 4x4: sum over density pairs of w (e_x e_y^T + e_y e_x^T)).
+  const double* pk; double MJ[16], MK[16];
   int nbf;
   double cK, cLR, omega2; int use_lr;
   double* grad;                    // [natom][3]

@@ -1,10 +1,11 @@
 // tdg_grad.cuh — per-class ERI-derivative + density-contraction kernel (steps a4-a8; Fig. 1).
 //
-// Work mapping (differs from Fig. 1's "1 thread = 1 batch"): a block work item is one bra tile of
-// 32 consecutive sorted shell pairs (one per lane) times a chunk of TDG_KB sorted ket pairs (TDG_KW per warp).
-// Every lane of a warp works on the SAME ket pair, so ket pair data are warp-uniform loads, the ket-centre
-// gradient is reduced with warp shuffles (1 atomic per 32 quartets), and the bra-centre gradient stays in
-// registers over the ket loop.  The fourth centre follows from translational invariance (eq 41).
+// Work mapping (differs from Fig. 1's "1 thread = 1 batch" over a dense supermatrix): a block work item
+// is one bra tile of 32 consecutive sorted shell pairs times a chunk of TDG_KB sorted ket pairs.  Phase 1 screens the
+// 32 x TDG_KB candidates (one ket per thread) and compacts the survivors into a shared-memory list; phase 2 processes
+// the survivors densely, one quartet per thread, so lanes do not idle on quartets the density-weighted test rejected.
+// Gradient contributions go to per-block shared-memory accumulators (one slot per bra/ket pair centre) that are flushed
+// with one FP64 atomic per touched slot.  The fourth centre follows from translational invariance (eq 41).
 //
 // Integrals: Rys quadrature: n_r = floor((L+1)/2)+1 roots (reading S6) for the full operator and
 // again for erf(omega r)/r (roots at s^2 T, x <- s^2 x, w <- s w; reading S8); 2-D recurrences of DESIGN.md
@@ -99,32 +100,57 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
   constexpr int NA = C::NA, NB = C::NB, NC = C::NC, ND = C::ND, NR = C::NR, U = C::UNR;
   constexpr bool SM = C::SMALL;
   double GF[C::NCOMP], GL[C::NCOMP];
-  {  // step a7, part 1: symmetrised density products for every function quartet
+  {  // step a7, part 1: symmetrised density products for every function quartet, from the packed blocks
+    //   Gt_K = u.MK.v + s.MK.t,  u = pk(ik)[a,c], v = pk(jl)[b,d], s = pk(jk)[b,c], t = pk(il)[a,d];  Gt_J = pk(ij)[a,b].MJ.pk(kl)[c,d]
     const size_t n = (size_t)P.nbf;
+    const double* __restrict__ pk = P.pk;
+    const double2* bIK = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offA * n + (size_t)NA * kh.offA));
+    const double2* bJL = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offB * n + (size_t)NB * kh.offB));
+    const double2* bJK = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offB * n + (size_t)NB * kh.offA));
+    const double2* bIL = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offA * n + (size_t)NA * kh.offB));
+    const double2* bIJ = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offA * n + (size_t)NA * bh.offB));
+    const double2* bKL = reinterpret_cast<const double2*>(pk + 4 * ((size_t)kh.offA * n + (size_t)NC * kh.offB));
+    // transformed small blocks: MK.v (jl), MK.t (il), MJ.(kl)
+    double vJL[NB * ND][4], tIL[NA * ND][4], vKL[NC * ND][4];
+#pragma unroll(U)
+    for (int e = 0; e < NB * ND; ++e) {
+      const double2 x0 = __ldg(bJL + 2 * e), x1 = __ldg(bJL + 2 * e + 1);
+#pragma unroll
+      for (int m = 0; m < 4; ++m) vJL[e][m] = P.MK[4 * m] * x0.x + P.MK[4 * m + 1] * x0.y + P.MK[4 * m + 2] * x1.x + P.MK[4 * m + 3] * x1.y;
+    }
+#pragma unroll(U)
+    for (int e = 0; e < NA * ND; ++e) {
+      const double2 x0 = __ldg(bIL + 2 * e), x1 = __ldg(bIL + 2 * e + 1);
+#pragma unroll
+      for (int m = 0; m < 4; ++m) tIL[e][m] = P.MK[4 * m] * x0.x + P.MK[4 * m + 1] * x0.y + P.MK[4 * m + 2] * x1.x + P.MK[4 * m + 3] * x1.y;
+    }
+#pragma unroll(U)
+    for (int e = 0; e < NC * ND; ++e) {
+      const double2 x0 = __ldg(bKL + 2 * e), x1 = __ldg(bKL + 2 * e + 1);
+#pragma unroll
+      for (int m = 0; m < 4; ++m) vKL[e][m] = P.MJ[4 * m] * x0.x + P.MJ[4 * m + 1] * x0.y + P.MJ[4 * m + 2] * x1.x + P.MJ[4 * m + 3] * x1.y;
+    }
 #pragma unroll(U)
     for (int a = 0; a < NA; ++a)
 #pragma unroll(U)
-      for (int b = 0; b < NB; ++b)
+      for (int b = 0; b < NB; ++b) {
+        const double2 j0 = __ldg(bIJ + 2 * (a * NB + b)), j1 = __ldg(bIJ + 2 * (a * NB + b) + 1);
 #pragma unroll(U)
-        for (int c = 0; c < NC; ++c)
+        for (int c = 0; c < NC; ++c) {
+          const double2 u0 = __ldg(bIK + 2 * (a * NC + c)), u1 = __ldg(bIK + 2 * (a * NC + c) + 1);
+          const double2 s0 = __ldg(bJK + 2 * (b * NC + c)), s1 = __ldg(bJK + 2 * (b * NC + c) + 1);
 #pragma unroll(U)
           for (int d = 0; d < ND; ++d) {
-            const size_t mu = bh.offA + a, nu = bh.offB + b, la = kh.offA + c, si = kh.offB + d;
-            double gj = 0.0, gk = 0.0;
-            for (int q = 0; q < P.nJ; ++q) {
-              const double* X = P.jp[q].X; const double* Y = P.jp[q].Y;
-              gj += P.jp[q].w * (__ldg(X + mu * n + nu) * __ldg(Y + la * n + si) + __ldg(X + la * n + si) * __ldg(Y + mu * n + nu));
-            }
-            for (int q = 0; q < P.nK; ++q) {
-              const double* X = P.kp[q].X; const double* Y = P.kp[q].Y;
-              gk += P.kp[q].w * (__ldg(X + mu * n + la) * __ldg(Y + nu * n + si) + __ldg(X + nu * n + la) * __ldg(Y + mu * n + si) +
-                                 __ldg(X + mu * n + si) * __ldg(Y + nu * n + la) + __ldg(X + nu * n + si) * __ldg(Y + mu * n + la));
-            }
+            const double* v = vJL[b * ND + d]; const double* tt = tIL[a * ND + d]; const double* w = vKL[c * ND + d];
+            const double gk = u0.x * v[0] + u0.y * v[1] + u1.x * v[2] + u1.y * v[3] + s0.x * tt[0] + s0.y * tt[1] + s1.x * tt[2] + s1.y * tt[3];
+            const double gj = j0.x * w[0] + j0.y * w[1] + j1.x * w[2] + j1.y * w[3];
             const double cn = deg * c_cnorm[LA][a] * c_cnorm[LB][b] * c_cnorm[LC][c] * c_cnorm[LD][d];
             const int idx = ((a * NB + b) * NC + c) * ND + d;
             GF[idx] = cn * (gj + P.cK * gk);
             GL[idx] = cn * P.cLR * gk;
           }
+        }
+      }
   }
 #pragma unroll
   for (int t = 0; t < 9; ++t) g[t] = 0.0;
@@ -201,88 +227,121 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
 
 __device__ __forceinline__ void red_add(double* addr, double v) { atomicAdd(addr, v); }
 
+#define TDG_NT (TDG_WARPS * TDG_WARP)
+
 template <int LA, int LB, int LC, int LD>
-__global__ void __launch_bounds__(TDG_WARPS * TDG_WARP) tdg_grad_kernel(const __grid_constant__ KParams P) {
+__global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant__ KParams P) {
+  __shared__ PairHdr s_bra[TDG_WARP];
+  __shared__ PairHdr s_ket[TDG_KB];
+  __shared__ double s_dij[TDG_WARP];
+  __shared__ double s_g[(TDG_WARP + TDG_KB) * 6];     // [pair][centre(2)][xyz]: bra pairs then ket pairs
+  __shared__ uint16_t s_list[TDG_WARP * TDG_KB];      // surviving quartets of this work item: ket_local << 5 | bra_local
+  __shared__ int s_wcnt[TDG_WARPS];
   // block work item -> (bra tile, ket chunk): largest t with cum[t] <= item
   const int item = blockIdx.x;
   int lo = 0, hi = P.ntiles;
   while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (__ldg(P.cum + mid) <= item) lo = mid; else hi = mid; }
   const int tile = lo, chunk = item - __ldg(P.cum + tile);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int bra = tile * TDG_WARP + lane;
-  const bool bra_ok = bra < P.nbra;
-  PairHdr bh = P.bra_hdr[bra_ok ? bra : P.nbra - 1];
-  const double* bprim = P.bra_prim + (size_t)(bra_ok ? bra : P.nbra - 1) * P.nppb * TDG_PRIM_STRIDE;
-  const int k0 = chunk * TDG_KB + warp * TDG_KW;
-  int k1 = k0 + TDG_KW; if (k1 > P.nket) k1 = P.nket;
-  double gA[3] = {0, 0, 0}, gB[3] = {0, 0, 0};
-  unsigned long long n_vis = 0, n_cmp = 0, n_prim = 0;
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
   const int ns = P.nshell;
-  for (int k = k0; k < k1; ++k) {
-    const PairHdr kh = P.ket_hdr[k];
-    bool act = bra_ok && (!P.same_bucket || k <= bra);
-    if (act && P.tau > 0.0) {   // step a4 (reading S9)
-      const double qq = bh.Q * kh.Q;
-      act = qq >= P.tau;
-      if (act) {
+  const int bra0 = tile * TDG_WARP, k0 = chunk * TDG_KB;
+  const int nb = min(TDG_WARP, P.nbra - bra0);
+  const bool dw = P.tau > 0.0 && P.density_weighted;
+  if (t < nb) {
+    const PairHdr h = P.bra_hdr[bra0 + t];
+    s_bra[t] = h;
+    s_dij[t] = dw ? __ldg(P.dmax + (size_t)h.ish * ns + h.jsh) : 0.0;
+  }
+  const int k = k0 + t;
+  const bool ket_ok = k < P.nket;
+  if (ket_ok) s_ket[t] = P.ket_hdr[k];
+  for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) s_g[i] = 0.0;
+  __syncthreads();
+  // ---- phase 1 (step a4; reading S9): one ket per thread, test it against the 32 bras ----
+  unsigned mask = 0;
+  unsigned long long n_vis = 0, n_cmp = 0;
+  if (ket_ok) {
+    const PairHdr& kh = s_ket[t];
+    const int ksh = kh.ish, lsh = kh.jsh;
+    const double Qk = kh.Q;
+    const double dkl = dw ? __ldg(P.dmax + (size_t)ksh * ns + lsh) : 0.0;
+    const bool ket_one = kh.atomA == kh.atomB;
+    for (int b = 0; b < nb; ++b) {
+      if (P.same_bucket && k > bra0 + b) continue;
+      const PairHdr& bh = s_bra[b];
+      if (P.tau > 0.0) {
+        const double qq = bh.Q * Qk;
+        if (!(qq >= P.tau)) continue;
         ++n_vis;
-        if (P.density_weighted) {
-          const double dij = __ldg(P.dmax + (size_t)bh.ish * ns + bh.jsh), dkl = __ldg(P.dmax + (size_t)kh.ish * ns + kh.jsh);
-          const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + kh.ish), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + kh.jsh);
-          const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + kh.jsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + kh.ish);
+        if (dw) {
+          const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + ksh), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + lsh);
+          const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + lsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + ksh);
           const double x1 = dik * djl, x2 = dil * djk;
-          double W = P.CJ * dij * dkl; const double WK = P.CK * (x1 > x2 ? x1 : x2);
+          double W = P.CJ * s_dij[b] * dkl; const double WK = P.CK * (x1 > x2 ? x1 : x2);
           if (WK > W) W = WK;
-          if (qq * W < P.tau) act = false;
+          if (qq * W < P.tau) continue;
         }
-      }
-    } else if (act) ++n_vis;
-    if (act && !tdg_sample_keep(bh.ish, bh.jsh, kh.ish, kh.jsh, P.sample_mod, P.sample_seed)) act = false;
-    if (act) {
-      ++n_cmp; n_prim += (unsigned long long)P.nppb * P.nppk;
+      } else ++n_vis;
+      if (!tdg_sample_keep(bh.ish, bh.jsh, ksh, lsh, P.sample_mod, P.sample_seed)) continue;
+      ++n_cmp;
       // all four shells on one atom: the four centre derivatives sum to zero on that atom (reading S11)
-      if (bh.atomA == bh.atomB && kh.atomA == kh.atomB && bh.atomA == kh.atomA) act = false;
-    }
-    if (!__any_sync(0xffffffffu, act)) continue;
-    double g[9];
-    if (act) {
-      double deg = 1.0;
-      if (bh.ish == bh.jsh) deg *= 0.5;
-      if (kh.ish == kh.jsh) deg *= 0.5;
-      if (P.same_bucket && k == bra) deg *= 0.5;
-      quartet_grad<LA, LB, LC, LD>(P, bh, bprim, kh, P.ket_prim + (size_t)k * P.nppk * TDG_PRIM_STRIDE, deg, g);
-    } else {
-#pragma unroll
-      for (int t = 0; t < 9; ++t) g[t] = 0.0;
-    }
-    // step a8: bra centres stay in registers; ket centres are reduced over the warp (all lanes share this ket)
-    double gC[3], gD[3];
-#pragma unroll
-    for (int x = 0; x < 3; ++x) {
-      gA[x] += g[x]; gB[x] += g[3 + x];
-      gC[x] = warp_sum(g[6 + x]);
-      gD[x] = -warp_sum(g[x] + g[3 + x] + g[6 + x]);
-    }
-    if (lane == 0) {
-#pragma unroll
-      for (int x = 0; x < 3; ++x) { red_add(P.grad + 3 * kh.atomA + x, gC[x]); red_add(P.grad + 3 * kh.atomB + x, gD[x]); }
+      if (ket_one && bh.atomA == bh.atomB && bh.atomA == kh.atomA) continue;
+      mask |= 1u << b;
     }
   }
-  if (bra_ok) {
+  // block-wide exclusive scan of the survivor counts -> compacted list, ket-major
+  const int cnt = __popc(mask);
+  int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+  if (lane == 31) s_wcnt[warp] = incl;
+  __syncthreads();
+  int off = incl - cnt, total = 0;
+#pragma unroll
+  for (int w = 0; w < TDG_WARPS; ++w) { const int c = s_wcnt[w]; if (w < warp) off += c; total += c; }
+  while (mask) { const int b = __ffs(mask) - 1; mask &= mask - 1; s_list[off++] = (uint16_t)((t << 5) | b); }
+  __syncthreads();
+  // ---- phase 2 (steps a5-a8): survivors are processed densely, one quartet per thread per pass ----
+  for (int s = t; s < total; s += TDG_NT) {
+    const unsigned e = s_list[s];
+    const int kt = e >> 5, b = e & 31;
+    const PairHdr& bh = s_bra[b];
+    const PairHdr& kh = s_ket[kt];
+    double deg = 1.0;
+    if (bh.ish == bh.jsh) deg *= 0.5;
+    if (kh.ish == kh.jsh) deg *= 0.5;
+    if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
+    double g[9];
+    quartet_grad<LA, LB, LC, LD>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
+                                 P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, g);
+    // step a8: block-level accumulators in shared memory; fourth centre by translational invariance (eq 41)
+    double* gb = s_g + b * 6;
+    double* gk = s_g + (TDG_WARP + kt) * 6;
 #pragma unroll
     for (int x = 0; x < 3; ++x) {
-      if (gA[x] != 0.0) red_add(P.grad + 3 * bh.atomA + x, gA[x]);
-      if (gB[x] != 0.0) red_add(P.grad + 3 * bh.atomB + x, gB[x]);
+      atomicAdd(gb + x, g[x]);
+      atomicAdd(gb + 3 + x, g[3 + x]);
+      atomicAdd(gk + x, g[6 + x]);
+      atomicAdd(gk + 3 + x, -(g[x] + g[3 + x] + g[6 + x]));
+    }
+  }
+  __syncthreads();
+  for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
+    const double v = s_g[i];
+    if (v != 0.0) {
+      const int pr = i / 6, r = i - pr * 6;
+      const PairHdr& h = pr < TDG_WARP ? s_bra[pr] : s_ket[pr - TDG_WARP];
+      red_add(P.grad + 3 * (r < 3 ? h.atomA : h.atomB) + (r < 3 ? r : r - 3), v);
     }
   }
   // stats
   for (int o = 16; o > 0; o >>= 1) {
     n_vis += __shfl_xor_sync(0xffffffffu, n_vis, o);
     n_cmp += __shfl_xor_sync(0xffffffffu, n_cmp, o);
-    n_prim += __shfl_xor_sync(0xffffffffu, n_prim, o);
   }
   if (lane == 0 && n_vis) {
-    atomicAdd(P.counters + 0, n_vis); atomicAdd(P.counters + 1, n_cmp); atomicAdd(P.counters + 2, n_prim);
+    atomicAdd(P.counters + 0, n_vis); atomicAdd(P.counters + 1, n_cmp);
+    atomicAdd(P.counters + 2, n_cmp * (unsigned long long)(P.nppb * P.nppk));
   }
 }
 

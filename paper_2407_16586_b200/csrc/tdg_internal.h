@@ -18,3 +18,9 @@ cudaError_t tdg_launch_symsplit(const double* M, int n, double* S, double* N, cu
 cudaError_t tdg_launch_dmax(const double* const* mats_dev, int nmat, int n, const DevShell* sh, int ns, double* m, cudaStream_t s);
 cudaError_t tdg_launch_rys(int n, int count, const double* T, const double* rho, double omega, const double* tab, double* out, cudaStream_t s);
 cudaError_t tdg_run_fp64_peak(double ms, double* tflops);
+
+// Packed density array (a3): shell-blocked, 4 canonical matrices interleaved.  For shells I (rows) and K (columns),
+// element (a, c) of canonical matrix m sits at pk[4*(off_I*nbf + n_I*off_K) + (a*n_K + c)*4 + m].  src[m] is an input
+// matrix (row-major, device) or nullptr (slot = 0); kind[m] = 0: symmetric part (M+M^T)/2, 1: antisymmetric part (M-M^T)/2.
+struct PackSrc { const double* src[4]; int kind[4]; };
+cudaError_t tdg_launch_pack(const PackSrc& ps, int n, const int* bf2sh, const DevShell* sh, double* pk, cudaStream_t s);
