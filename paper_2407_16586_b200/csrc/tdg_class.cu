@@ -9,7 +9,7 @@
 
 template <int LC, int LD>
 static void launch(const KParams& P, int nblocks, cudaStream_t s) {
-  tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD><<<nblocks, TDG_WARPS * TDG_WARP, 0, s>>>(P);
+  tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD><<<dim3(nblocks, QC<TDG_LA, TDG_LB, LC, LD>::NROLE), TDG_WARPS * TDG_WARP, 0, s>>>(P);
 }
 template <int LC, int LD>
 static tdg_launch_fn pick() {

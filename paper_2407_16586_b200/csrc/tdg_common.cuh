@@ -54,6 +54,13 @@ __host__ __device__ constexpr int cart_exp(int l, int idx, int d) {
     }
   return 0;
 }
+// the same, forced to compile time: 4 bits per component packed into one constant (cheap to fold after unrolling)
+__host__ __device__ constexpr unsigned long long cart_pack(int l, int d) {
+  unsigned long long v = 0;
+  for (int i = 0; i < ncart(l); ++i) v |= (unsigned long long)cart_exp(l, i, d) << (4 * i);
+  return v;
+}
+template <int L, int D> struct CartPack { static constexpr unsigned long long v = cart_pack(L, D); };
 // packed runtime table: [l][idx] -> lx | ly<<4 | lz<<8
 __constant__ static uint16_t c_cart[4][10] = {
   {0x000},

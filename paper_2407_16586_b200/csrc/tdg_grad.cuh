@@ -14,6 +14,13 @@
 // symmetrised density product Gt (eqs 13-14) and accumulated into 9 scalars.
 #pragma once
 #include "tdg_common.cuh"
+#define TDG_NT (TDG_WARPS * TDG_WARP)
+#ifndef TDG_RU_LIM
+#define TDG_RU_LIM 120
+#endif
+#ifndef TDG_MAX_ROLES
+#define TDG_MAX_ROLES 6   // classes needing more roles keep rolled loops (compile time)
+#endif
 
 template <int LA, int LB, int LC, int LD>
 struct QC {
@@ -23,8 +30,18 @@ struct QC {
   static constexpr int NR = (L + 1) / 2 + 1;
   static constexpr int DA = LA + 2, DB = LB + 2, DC = LC + 2, DD = LD + 1;
   static constexpr int NMX = LA + LB + 1, MMX = LC + LD + 1;
-  static constexpr bool SMALL = NCOMP <= 27;
+  // Component slicing ("roles", grid.y): a block of role r handles the bra function pairs ab in [r*ABN, (r+1)*ABN) of
+  // every surviving quartet, so that a thread holds at most ~27 density products and fully unrolled code stays in
+  // registers; the 2-D integrals are rebuilt by every role.  Classes with an f shell keep rolled loops (one role).
+  static constexpr bool HASF = LA == 3 || LB == 3 || LC == 3 || LD == 3;
+  static constexpr int NAB = NA * NB, KDN = NC * ND;
+  static constexpr int ABN1 = 27 / KDN >= NAB ? NAB : (27 / KDN > 0 ? 27 / KDN : 1);
+  static constexpr int NROLE1 = (NAB + ABN1 - 1) / ABN1;
+  static constexpr bool SMALL = NCOMP <= 27 || (!HASF && NROLE1 <= TDG_MAX_ROLES);   // fully unrolled code
+  static constexpr int NROLE = SMALL ? NROLE1 : 1;
+  static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;
+  static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
 };
 
 // 2-D integrals of one direction for one root: I[i][j][k][l], i<=LA+1, j<=LB+1 (i+j<=LA+LB+1), k<=LC+1, l<=LD.
@@ -86,20 +103,23 @@ __device__ __forceinline__ void build2d(double c00, double c00p, double b00, dou
 
 template <int L, bool SMALL>
 __device__ __forceinline__ void comp_exps(int idx, int& x, int& y, int& z) {
-  if (SMALL) { x = cart_exp(L, idx, 0); y = cart_exp(L, idx, 1); z = cart_exp(L, idx, 2); }
+  if (SMALL) {
+    x = (int)((CartPack<L, 0>::v >> (4 * idx)) & 15); y = (int)((CartPack<L, 1>::v >> (4 * idx)) & 15); z = (int)((CartPack<L, 2>::v >> (4 * idx)) & 15);
+  }
   else { unsigned v = c_cart[L][idx]; x = v & 15; y = (v >> 4) & 15; z = (v >> 8) & 15; }
 }
 
 // Gradient contribution of one shell quartet: g[0..2] = d/dA, g[3..5] = d/dB, g[6..8] = d/dC (sum over all
 // functions, primitives, roots and both operators, already multiplied by deg and the density products).
-template <int LA, int LB, int LC, int LD>
+template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh, const double* __restrict__ bprim,
                                              const PairHdr& kh, const double* __restrict__ kprim, double deg,
                                              double (&g)[9]) {
   typedef QC<LA, LB, LC, LD> C;
-  constexpr int NA = C::NA, NB = C::NB, NC = C::NC, ND = C::ND, NR = C::NR, U = C::UNR;
+  constexpr int NA = C::NA, NB = C::NB, NC = C::NC, ND = C::ND, NR = C::NR, U = C::UNR, RU = C::RUNR;
   constexpr bool SM = C::SMALL;
-  double GF[C::NCOMP], GL[C::NCOMP];
+  // this role's bra function pairs: ab = a*NB + b in [AB0, AB0+ABC)
+  double GF[ABC * NC * ND], GL[ABC * NC * ND];
   {  // step a7, part 1: symmetrised density products for every function quartet, from the packed blocks
     //   Gt_K = u.MK.v + s.MK.t,  u = pk(ik)[a,c], v = pk(jl)[b,d], s = pk(jk)[b,c], t = pk(il)[a,d];  Gt_J = pk(ij)[a,b].MJ.pk(kl)[c,d]
     const size_t n = (size_t)P.nbf;
@@ -131,9 +151,9 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
       for (int m = 0; m < 4; ++m) vKL[e][m] = P.MJ[4 * m] * x0.x + P.MJ[4 * m + 1] * x0.y + P.MJ[4 * m + 2] * x1.x + P.MJ[4 * m + 3] * x1.y;
     }
 #pragma unroll(U)
-    for (int a = 0; a < NA; ++a)
-#pragma unroll(U)
-      for (int b = 0; b < NB; ++b) {
+    for (int ab = AB0; ab < AB0 + ABC; ++ab) {
+      {
+        const int a = ab / NB, b = ab - a * NB;
         const double2 j0 = __ldg(bIJ + 2 * (a * NB + b)), j1 = __ldg(bIJ + 2 * (a * NB + b) + 1);
 #pragma unroll(U)
         for (int c = 0; c < NC; ++c) {
@@ -145,12 +165,13 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
             const double gk = u0.x * v[0] + u0.y * v[1] + u1.x * v[2] + u1.y * v[3] + s0.x * tt[0] + s0.y * tt[1] + s1.x * tt[2] + s1.y * tt[3];
             const double gj = j0.x * w[0] + j0.y * w[1] + j1.x * w[2] + j1.y * w[3];
             const double cn = deg * c_cnorm[LA][a] * c_cnorm[LB][b] * c_cnorm[LC][c] * c_cnorm[LD][d];
-            const int idx = ((a * NB + b) * NC + c) * ND + d;
+            const int idx = ((ab - AB0) * NC + c) * ND + d;
             GF[idx] = cn * (gj + P.cK * gk);
             GL[idx] = cn * P.cLR * gk;
           }
         }
       }
+    }
   }
 #pragma unroll
   for (int t = 0; t < 9; ++t) g[t] = 0.0;
@@ -175,7 +196,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
         double xr[NR], wr[NR];
         rys_roots<NR>(P.rys_tab, s2 * T, xr, wr);
         const double* __restrict__ G = op == 0 ? GF : GL;
-#pragma unroll(U)
+#pragma unroll(RU)
         for (int r = 0; r < NR; ++r) {
           const double x = xr[r] * s2, w = wr[r] * ss * pref;
           const double b00 = 0.5 * x * rpq, b10 = (0.5 - q * b00) * rp, b01 = (0.5 - p * b00) * rq;
@@ -186,10 +207,10 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
           build2d<LA, LB, LC, LD>(PAz - fq * PQz, QCz + fp * PQz, b00, b10, b01, ABz, CDz, w, Iz);
           // step a7, part 2: contract the derivative integrals of this root with Gt
 #pragma unroll(U)
-          for (int a = 0; a < NA; ++a) {
+          for (int ab = AB0; ab < AB0 + ABC; ++ab) {
+            const int a = ab / NB, b = ab - a * NB;
             int ax, ay, az; comp_exps<LA, SM>(a, ax, ay, az);
-#pragma unroll(U)
-            for (int b = 0; b < NB; ++b) {
+            {
               int bx, by, bz; comp_exps<LB, SM>(b, bx, by, bz);
 #pragma unroll(U)
               for (int c = 0; c < NC; ++c) {
@@ -197,7 +218,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
 #pragma unroll(U)
                 for (int d = 0; d < ND; ++d) {
                   int dx, dy, dz; comp_exps<LD, SM>(d, dx, dy, dz);
-                  const double Gv = G[((a * NB + b) * NC + c) * ND + d];
+                  const double Gv = G[((ab - AB0) * NC + c) * ND + d];
                   const double X0 = Ix[ax][bx][cx][dx], Y0 = Iy[ay][by][cy][dy], Z0 = Iz[az][bz][cz][dz];
                   const double tx = Gv * Y0 * Z0, ty = Gv * X0 * Z0, tz = Gv * X0 * Y0;
                   double dAx = a2 * Ix[ax + 1][bx][cx][dx], dAy = a2 * Iy[ay + 1][by][cy][dy], dAz = a2 * Iz[az + 1][bz][cz][dz];
@@ -225,9 +246,50 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
   }
 }
 
+// Phase 2 of the kernel for one role (slice [AB0, AB0+ABC) of the bra function pairs).
+template <int LA, int LB, int LC, int LD, int AB0, int ABC>
+__device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
+                                                  const uint16_t* s_list, double* s_g, int total, int bra0, int k0) {
+  for (int s = threadIdx.x; s < total; s += TDG_NT) {
+    const unsigned e = s_list[s];
+    const int kt = e >> 5, b = e & 31;
+    const PairHdr& bh = s_bra[b];
+    const PairHdr& kh = s_ket[kt];
+    double deg = 1.0;
+    if (bh.ish == bh.jsh) deg *= 0.5;
+    if (kh.ish == kh.jsh) deg *= 0.5;
+    if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
+    double g[9];
+    quartet_grad<LA, LB, LC, LD, AB0, ABC>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
+                                           P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, g);
+    // step a8: block-level accumulators in shared memory; fourth centre by translational invariance (eq 41)
+    double* gb = s_g + b * 6;
+    double* gk = s_g + (TDG_WARP + kt) * 6;
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+      atomicAdd(gb + x, g[x]);
+      atomicAdd(gb + 3 + x, g[3 + x]);
+      atomicAdd(gk + x, g[6 + x]);
+      atomicAdd(gk + 3 + x, -(g[x] + g[3 + x] + g[6 + x]));
+    }
+  }
+}
+template <int LA, int LB, int LC, int LD, int R>
+struct RoleDispatch {
+  typedef QC<LA, LB, LC, LD> C;
+  static __device__ __forceinline__ void run(int role, const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
+                                             const uint16_t* s_list, double* s_g, int total, int bra0, int k0) {
+    if constexpr (R < C::NROLE) {
+      constexpr int AB0 = R * C::ABN;
+      constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
+      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, s_list, s_g, total, bra0, k0);
+      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, s_list, s_g, total, bra0, k0);
+    }
+  }
+};
+
 __device__ __forceinline__ void red_add(double* addr, double v) { atomicAdd(addr, v); }
 
-#define TDG_NT (TDG_WARPS * TDG_WARP)
 
 template <int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant__ KParams P) {
@@ -302,29 +364,7 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   while (mask) { const int b = __ffs(mask) - 1; mask &= mask - 1; s_list[off++] = (uint16_t)((t << 5) | b); }
   __syncthreads();
   // ---- phase 2 (steps a5-a8): survivors are processed densely, one quartet per thread per pass ----
-  for (int s = t; s < total; s += TDG_NT) {
-    const unsigned e = s_list[s];
-    const int kt = e >> 5, b = e & 31;
-    const PairHdr& bh = s_bra[b];
-    const PairHdr& kh = s_ket[kt];
-    double deg = 1.0;
-    if (bh.ish == bh.jsh) deg *= 0.5;
-    if (kh.ish == kh.jsh) deg *= 0.5;
-    if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
-    double g[9];
-    quartet_grad<LA, LB, LC, LD>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
-                                 P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, g);
-    // step a8: block-level accumulators in shared memory; fourth centre by translational invariance (eq 41)
-    double* gb = s_g + b * 6;
-    double* gk = s_g + (TDG_WARP + kt) * 6;
-#pragma unroll
-    for (int x = 0; x < 3; ++x) {
-      atomicAdd(gb + x, g[x]);
-      atomicAdd(gb + 3 + x, g[3 + x]);
-      atomicAdd(gk + x, g[6 + x]);
-      atomicAdd(gk + 3 + x, -(g[x] + g[3 + x] + g[6 + x]));
-    }
-  }
+  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, s_list, s_g, total, bra0, k0);
   __syncthreads();
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
     const double v = s_g[i];
@@ -339,7 +379,7 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
     n_vis += __shfl_xor_sync(0xffffffffu, n_vis, o);
     n_cmp += __shfl_xor_sync(0xffffffffu, n_cmp, o);
   }
-  if (lane == 0 && n_vis) {
+  if (lane == 0 && n_vis && blockIdx.y == 0) {
     atomicAdd(P.counters + 0, n_vis); atomicAdd(P.counters + 1, n_cmp);
     atomicAdd(P.counters + 2, n_cmp * (unsigned long long)(P.nppb * P.nppk));
   }
