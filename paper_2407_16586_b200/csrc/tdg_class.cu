@@ -9,7 +9,14 @@
 
 template <int LC, int LD>
 static void launch(const KParams& P, int nblocks, cudaStream_t s) {
-  tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD><<<dim3(nblocks, QC<TDG_LA, TDG_LB, LC, LD>::NROLE), TDG_WARPS * TDG_WARP, 0, s>>>(P);
+  typedef QC<TDG_LA, TDG_LB, LC, LD> C;
+  constexpr int smem = C::RYS_SH_DOUBLES * (int)sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set && smem > 0) {
+    cudaFuncSetAttribute(tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    attr_set = true;
+  }
+  tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD><<<dim3(nblocks, C::NROLE), TDG_WARPS * TDG_WARP, smem, s>>>(P);
 }
 template <int LC, int LD>
 static tdg_launch_fn pick() {

@@ -99,8 +99,11 @@ __host__ __device__ inline bool tdg_sample_keep(int i, int j, int k, int l, uint
 // Table layout (rys_tables.inc): for n: [interval][power, highest first][2n]; constants in __constant__.
 #include "rys_meta.inc"
 
+// `tabN` points at the table of this N (global: tab + rys_off(N); or a copy of it staged in shared memory, where the
+// lanes' different intervals cost bank conflicts instead of one L1 wavefront per lane).
+#define RYS_TABLE_DOUBLES(N) (rys_tmax(N) * (RYS_DEG + 1) * 2 * (N))
 template <int N>
-__device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double T, double* __restrict__ x, double* __restrict__ w) {
+__device__ __forceinline__ void rys_roots_tab(const double* __restrict__ tabN, double T, double* __restrict__ x, double* __restrict__ w) {
   if (T >= (double)rys_tmax(N)) {
     double rT = 1.0 / T, rs = sqrt(rT);
 #pragma unroll
@@ -109,17 +112,25 @@ __device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double
   }
   int i = (int)T;                       // RYS_H == 1
   double u = (T - ((double)i + 0.5)) * 2.0;
-  const double* c = tab + rys_off(N) + i * ((RYS_DEG + 1) * 2 * N);
-  double v[2 * N];
+  const double2* c = reinterpret_cast<const double2*>(tabN + i * ((RYS_DEG + 1) * 2 * N));   // rows of 2N doubles: 16-byte aligned
+  double2 v[N];
 #pragma unroll
-  for (int f = 0; f < 2 * N; ++f) v[f] = __ldg(c + f);
+  for (int f = 0; f < N; ++f) v[f] = c[f];
 #pragma unroll
   for (int k = 1; k <= RYS_DEG; ++k) {
 #pragma unroll
-    for (int f = 0; f < 2 * N; ++f) v[f] = fma(v[f], u, __ldg(c + k * 2 * N + f));
+    for (int f = 0; f < N; ++f) { const double2 ck = c[k * N + f]; v[f].x = fma(v[f].x, u, ck.x); v[f].y = fma(v[f].y, u, ck.y); }
   }
+  // row layout: x_0..x_{N-1}, w_0..w_{N-1}
 #pragma unroll
-  for (int r = 0; r < N; ++r) { x[r] = v[r]; w[r] = v[N + r]; }
+  for (int r = 0; r < N; ++r) {
+    x[r] = (r & 1) ? v[r >> 1].y : v[r >> 1].x;
+    w[r] = ((N + r) & 1) ? v[(N + r) >> 1].y : v[(N + r) >> 1].x;
+  }
+}
+template <int N>
+__device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double T, double* __restrict__ x, double* __restrict__ w) {
+  rys_roots_tab<N>(tab + rys_off(N), T, x, w);
 }
 
 __device__ __forceinline__ double warp_sum(double v) {

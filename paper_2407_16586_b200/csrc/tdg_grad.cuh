@@ -41,6 +41,8 @@ struct QC {
   static constexpr int NROLE = SMALL ? NROLE1 : 1;
   static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;
+  static constexpr bool RYS_SH = NR <= 4;                                  // Rys table of this NR staged in shared memory
+  static constexpr int RYS_SH_DOUBLES = RYS_SH ? RYS_TABLE_DOUBLES(NR) : 0;
   static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
 };
 
@@ -114,7 +116,7 @@ __device__ __forceinline__ void comp_exps(int idx, int& x, int& y, int& z) {
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh, const double* __restrict__ bprim,
                                              const PairHdr& kh, const double* __restrict__ kprim, double deg,
-                                             double (&g)[9]) {
+                                             const double* __restrict__ rys, double (&g)[9]) {
   typedef QC<LA, LB, LC, LD> C;
   constexpr int NA = C::NA, NB = C::NB, NC = C::NC, ND = C::ND, NR = C::NR, U = C::UNR, RU = C::RUNR;
   constexpr bool SM = C::SMALL;
@@ -194,7 +196,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
         double s2 = 1.0, ss = 1.0;
         if (op == 1) { s2 = P.omega2 / (P.omega2 + rho); ss = sqrt(s2); }
         double xr[NR], wr[NR];
-        rys_roots<NR>(P.rys_tab, s2 * T, xr, wr);
+        rys_roots_tab<NR>(rys, s2 * T, xr, wr);
         const double* __restrict__ G = op == 0 ? GF : GL;
 #pragma unroll(RU)
         for (int r = 0; r < NR; ++r) {
@@ -249,10 +251,26 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
 // Phase 2 of the kernel for one role (slice [AB0, AB0+ABC) of the bra function pairs).
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
-                                                  const uint16_t* s_list, double* s_g, int total, int bra0, int k0) {
-  for (int s = threadIdx.x; s < total; s += TDG_NT) {
+                                                  const uint16_t* s_list, double* s_g, int total, int bra0, int k0, const double* __restrict__ rys) {
+  // Each thread takes a contiguous run of the ket-major survivor list, so its consecutive quartets share the ket: the
+  // ket-centre gradient stays in registers until the ket changes, and the lanes of a warp work on different kets
+  // (no same-address conflicts in the shared-memory accumulators, which are CAS loops for FP64).
+  const int m = (total + TDG_NT - 1) / TDG_NT;
+  const int s0 = threadIdx.x * m;
+  const int s1 = min(s0 + m, total);
+  int cur = -1;
+  double kC[3] = {0.0, 0.0, 0.0}, kD[3] = {0.0, 0.0, 0.0};
+  for (int s = s0; s < s1; ++s) {
     const unsigned e = s_list[s];
     const int kt = e >> 5, b = e & 31;
+    if (kt != cur) {
+      if (cur >= 0) {
+        double* gk = s_g + (TDG_WARP + cur) * 6;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { atomicAdd(gk + x, kC[x]); atomicAdd(gk + 3 + x, kD[x]); kC[x] = 0.0; kD[x] = 0.0; }
+      }
+      cur = kt;
+    }
     const PairHdr& bh = s_bra[b];
     const PairHdr& kh = s_ket[kt];
     double deg = 1.0;
@@ -261,29 +279,33 @@ __device__ __forceinline__ void process_survivors(const KParams& P, const PairHd
     if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
     double g[9];
     quartet_grad<LA, LB, LC, LD, AB0, ABC>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
-                                           P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, g);
+                                           P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys, g);
     // step a8: block-level accumulators in shared memory; fourth centre by translational invariance (eq 41)
     double* gb = s_g + b * 6;
-    double* gk = s_g + (TDG_WARP + kt) * 6;
 #pragma unroll
     for (int x = 0; x < 3; ++x) {
       atomicAdd(gb + x, g[x]);
       atomicAdd(gb + 3 + x, g[3 + x]);
-      atomicAdd(gk + x, g[6 + x]);
-      atomicAdd(gk + 3 + x, -(g[x] + g[3 + x] + g[6 + x]));
+      kC[x] += g[6 + x];
+      kD[x] -= g[x] + g[3 + x] + g[6 + x];
     }
+  }
+  if (cur >= 0) {
+    double* gk = s_g + (TDG_WARP + cur) * 6;
+#pragma unroll
+    for (int x = 0; x < 3; ++x) { atomicAdd(gk + x, kC[x]); atomicAdd(gk + 3 + x, kD[x]); }
   }
 }
 template <int LA, int LB, int LC, int LD, int R>
 struct RoleDispatch {
   typedef QC<LA, LB, LC, LD> C;
   static __device__ __forceinline__ void run(int role, const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
-                                             const uint16_t* s_list, double* s_g, int total, int bra0, int k0) {
+                                             const uint16_t* s_list, double* s_g, int total, int bra0, int k0, const double* __restrict__ rys) {
     if constexpr (R < C::NROLE) {
       constexpr int AB0 = R * C::ABN;
       constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
-      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, s_list, s_g, total, bra0, k0);
-      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, s_list, s_g, total, bra0, k0);
+      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, s_list, s_g, total, bra0, k0, rys);
+      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, s_list, s_g, total, bra0, k0, rys);
     }
   }
 };
@@ -299,6 +321,8 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   __shared__ double s_g[(TDG_WARP + TDG_KB) * 6];     // [pair][centre(2)][xyz]: bra pairs then ket pairs
   __shared__ uint16_t s_list[TDG_WARP * TDG_KB];      // surviving quartets of this work item: ket_local << 5 | bra_local
   __shared__ int s_wcnt[TDG_WARPS];
+  extern __shared__ double2 s_rys[];                  // Rys table of this class (QC::RYS_SH)
+  typedef QC<LA, LB, LC, LD> C;
   // block work item -> (bra tile, ket chunk): largest t with cum[t] <= item
   const int item = blockIdx.x;
   int lo = 0, hi = P.ntiles;
@@ -318,6 +342,12 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   const bool ket_ok = k < P.nket;
   if (ket_ok) s_ket[t] = P.ket_hdr[k];
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) s_g[i] = 0.0;
+  const double* rys = P.rys_tab + rys_off(C::NR);
+  if (C::RYS_SH) {
+    const double2* src = reinterpret_cast<const double2*>(rys);
+    for (int i = t; i < C::RYS_SH_DOUBLES / 2; i += TDG_NT) s_rys[i] = __ldg(src + i);
+    rys = reinterpret_cast<const double*>(s_rys);
+  }
   __syncthreads();
   // ---- phase 1 (step a4; reading S9): one ket per thread, test it against the 32 bras ----
   unsigned mask = 0;
@@ -364,7 +394,7 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   while (mask) { const int b = __ffs(mask) - 1; mask &= mask - 1; s_list[off++] = (uint16_t)((t << 5) | b); }
   __syncthreads();
   // ---- phase 2 (steps a5-a8): survivors are processed densely, one quartet per thread per pass ----
-  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, s_list, s_g, total, bra0, k0);
+  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, s_list, s_g, total, bra0, k0, rys);
   __syncthreads();
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
     const double v = s_g[i];
