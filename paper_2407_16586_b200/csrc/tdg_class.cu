@@ -10,7 +10,7 @@
 template <int LC, int LD>
 static void launch(const KParams& P, int nblocks, cudaStream_t s) {
   typedef QC<TDG_LA, TDG_LB, LC, LD> C;
-  constexpr int smem = C::RYS_SH_DOUBLES * (int)sizeof(double);
+  constexpr int smem = (C::RYS_SH_DOUBLES + TDG_ACC_DOUBLES) * (int)sizeof(double);
   static bool attr_set = false;
   if (!attr_set && smem > 0) {
     cudaFuncSetAttribute(tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);

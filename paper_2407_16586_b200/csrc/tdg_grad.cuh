@@ -15,6 +15,7 @@
 #pragma once
 #include "tdg_common.cuh"
 #define TDG_NT (TDG_WARPS * TDG_WARP)
+#define TDG_ACC_DOUBLES (TDG_WARPS * (TDG_WARP + TDG_KB) * 6)
 #ifndef TDG_RU_LIM
 #define TDG_RU_LIM 120
 #endif
@@ -248,69 +249,81 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
   }
 }
 
+__device__ __forceinline__ void red_add(double* addr, double v) { atomicAdd(addr, v); }
+
 // Phase 2 of the kernel for one role (slice [AB0, AB0+ABC) of the bra function pairs).
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
-                                                  const uint16_t* s_list, double* s_g, int total, int bra0, int k0, const double* __restrict__ rys) {
-  // Each thread takes a contiguous run of the ket-major survivor list, so its consecutive quartets share the ket: the
-  // ket-centre gradient stays in registers until the ket changes, and the lanes of a warp work on different kets
-  // (no same-address conflicts in the shared-memory accumulators, which are CAS loops for FP64).
-  const int m = (total + TDG_NT - 1) / TDG_NT;
-  const int s0 = threadIdx.x * m;
-  const int s1 = min(s0 + m, total);
-  int cur = -1;
-  double kC[3] = {0.0, 0.0, 0.0}, kD[3] = {0.0, 0.0, 0.0};
-  for (int s = s0; s < s1; ++s) {
-    const unsigned e = s_list[s];
+                                                  const uint16_t* s_list, double* s_gb, double* s_gk, int total, int bra0, int k0, const double* __restrict__ rys) {
+  // Each warp takes passes of 32 consecutive entries of the ket-major survivor list.  Gradient accumulation uses no
+  // atomics (shared-memory FP64 atomics are CAS loops of ~60 iterations per warp and 6 RED per quartet saturate L2;
+  // both measured): lanes with the same ket are contiguous, so the ket-centre terms are summed by a segmented warp
+  // shuffle scan and added by the segment head to this warp's private slot; the bra-centre terms are added to this
+  // warp's private slots segment by segment (bras are distinct within a segment).  Fourth centre: eq 41.
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double* my_gb = s_gb + warp * (TDG_WARP * 6);
+  double* my_gk = s_gk + warp * (TDG_KB * 6);
+  for (int base = warp * TDG_WARP; base < total; base += TDG_NT) {
+    const int s = base + lane;
+    const bool act = s < total;
+    const unsigned e = act ? s_list[s] : 0u;
     const int kt = e >> 5, b = e & 31;
-    if (kt != cur) {
-      if (cur >= 0) {
-        double* gk = s_g + (TDG_WARP + cur) * 6;
-#pragma unroll
-        for (int x = 0; x < 3; ++x) { atomicAdd(gk + x, kC[x]); atomicAdd(gk + 3 + x, kD[x]); kC[x] = 0.0; kD[x] = 0.0; }
-      }
-      cur = kt;
-    }
-    const PairHdr& bh = s_bra[b];
-    const PairHdr& kh = s_ket[kt];
-    double deg = 1.0;
-    if (bh.ish == bh.jsh) deg *= 0.5;
-    if (kh.ish == kh.jsh) deg *= 0.5;
-    if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
     double g[9];
-    quartet_grad<LA, LB, LC, LD, AB0, ABC>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
-                                           P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys, g);
-    // step a8: block-level accumulators in shared memory; fourth centre by translational invariance (eq 41)
-    double* gb = s_g + b * 6;
+    if (act) {
+      const PairHdr& bh = s_bra[b];
+      const PairHdr& kh = s_ket[kt];
+      double deg = 1.0;
+      if (bh.ish == bh.jsh) deg *= 0.5;
+      if (kh.ish == kh.jsh) deg *= 0.5;
+      if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
+      quartet_grad<LA, LB, LC, LD, AB0, ABC>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
+                                             P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys, g);
+    } else {
 #pragma unroll
-    for (int x = 0; x < 3; ++x) {
-      atomicAdd(gb + x, g[x]);
-      atomicAdd(gb + 3 + x, g[3 + x]);
-      kC[x] += g[6 + x];
-      kD[x] -= g[x] + g[3 + x] + g[6 + x];
+      for (int x = 0; x < 9; ++x) g[x] = 0.0;
     }
-  }
-  if (cur >= 0) {
-    double* gk = s_g + (TDG_WARP + cur) * 6;
+    const int key = act ? kt : -1 - lane;
+    double v[6];
 #pragma unroll
-    for (int x = 0; x < 3; ++x) { atomicAdd(gk + x, kC[x]); atomicAdd(gk + 3 + x, kD[x]); }
+    for (int x = 0; x < 3; ++x) { v[x] = g[6 + x]; v[3 + x] = -(g[x] + g[3 + x] + g[6 + x]); }
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int ko = __shfl_down_sync(0xffffffffu, key, o);
+      const bool same = (lane + o < 32) && (ko == key);
+#pragma unroll
+      for (int x = 0; x < 6; ++x) { const double tv = __shfl_down_sync(0xffffffffu, v[x], o); if (same) v[x] += tv; }
+    }
+    const int kprev = __shfl_up_sync(0xffffffffu, key, 1);
+    const bool head = (lane == 0) || (kprev != key);
+    if (act && head) {
+#pragma unroll
+      for (int x = 0; x < 6; ++x) my_gk[kt * 6 + x] += v[x];
+    }
+    const unsigned hm = __ballot_sync(0xffffffffu, head);
+    const int seg = __popc(hm & (0xffffffffu >> (31 - lane))) - 1, nseg = __popc(hm);
+    for (int sidx = 0; sidx < nseg; ++sidx) {
+      if (act && seg == sidx) {
+#pragma unroll
+        for (int x = 0; x < 6; ++x) my_gb[b * 6 + x] += g[x];
+      }
+      __syncwarp();
+    }
   }
 }
 template <int LA, int LB, int LC, int LD, int R>
 struct RoleDispatch {
   typedef QC<LA, LB, LC, LD> C;
   static __device__ __forceinline__ void run(int role, const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
-                                             const uint16_t* s_list, double* s_g, int total, int bra0, int k0, const double* __restrict__ rys) {
+                                             const uint16_t* s_list, double* s_gb, double* s_gk, int total, int bra0, int k0, const double* __restrict__ rys) {
     if constexpr (R < C::NROLE) {
       constexpr int AB0 = R * C::ABN;
       constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
-      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, s_list, s_g, total, bra0, k0, rys);
-      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, s_list, s_g, total, bra0, k0, rys);
+      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, s_list, s_gb, s_gk, total, bra0, k0, rys);
+      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, s_list, s_gb, s_gk, total, bra0, k0, rys);
     }
   }
 };
 
-__device__ __forceinline__ void red_add(double* addr, double v) { atomicAdd(addr, v); }
 
 
 template <int LA, int LB, int LC, int LD>
@@ -318,11 +331,14 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   __shared__ PairHdr s_bra[TDG_WARP];
   __shared__ PairHdr s_ket[TDG_KB];
   __shared__ double s_dij[TDG_WARP];
-  __shared__ double s_g[(TDG_WARP + TDG_KB) * 6];     // [pair][centre(2)][xyz]: bra pairs then ket pairs
   __shared__ uint16_t s_list[TDG_WARP * TDG_KB];      // surviving quartets of this work item: ket_local << 5 | bra_local
   __shared__ int s_wcnt[TDG_WARPS];
-  extern __shared__ double2 s_rys[];                  // Rys table of this class (QC::RYS_SH)
+  // dynamic shared memory: per-warp private accumulators, then the Rys table of this class (QC::RYS_SH)
+  extern __shared__ double2 s_dyn[];
   typedef QC<LA, LB, LC, LD> C;
+  double* s_gb = reinterpret_cast<double*>(s_dyn);            // [warp][bra][centre A,B][xyz]
+  double* s_gk = s_gb + TDG_WARPS * TDG_WARP * 6;             // [warp][ket][centre C,D][xyz]
+  double2* s_rys = s_dyn + TDG_ACC_DOUBLES / 2;
   // block work item -> (bra tile, ket chunk): largest t with cum[t] <= item
   const int item = blockIdx.x;
   int lo = 0, hi = P.ntiles;
@@ -341,7 +357,8 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   const int k = k0 + t;
   const bool ket_ok = k < P.nket;
   if (ket_ok) s_ket[t] = P.ket_hdr[k];
-  for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) s_g[i] = 0.0;
+  for (int i = t; i < TDG_WARPS * TDG_WARP * 6; i += TDG_NT) s_gb[i] = 0.0;
+  for (int i = t; i < TDG_WARPS * TDG_KB * 6; i += TDG_NT) s_gk[i] = 0.0;
   const double* rys = P.rys_tab + rys_off(C::NR);
   if (C::RYS_SH) {
     const double2* src = reinterpret_cast<const double2*>(rys);
@@ -394,15 +411,24 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   while (mask) { const int b = __ffs(mask) - 1; mask &= mask - 1; s_list[off++] = (uint16_t)((t << 5) | b); }
   __syncthreads();
   // ---- phase 2 (steps a5-a8): survivors are processed densely, one quartet per thread per pass ----
-  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, s_list, s_g, total, bra0, k0, rys);
+  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, s_list, s_gb, s_gk, total, bra0, k0, rys);
   __syncthreads();
+  // flush: sum the warps' private slots, one FP64 RED per touched (pair, centre, xyz)
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
-    const double v = s_g[i];
-    if (v != 0.0) {
-      const int pr = i / 6, r = i - pr * 6;
-      const PairHdr& h = pr < TDG_WARP ? s_bra[pr] : s_ket[pr - TDG_WARP];
-      red_add(P.grad + 3 * (r < 3 ? h.atomA : h.atomB) + (r < 3 ? r : r - 3), v);
+    double v = 0.0;
+    const PairHdr* h;
+    int r;
+    if (i < TDG_WARP * 6) {
+#pragma unroll
+      for (int w = 0; w < TDG_WARPS; ++w) v += s_gb[w * (TDG_WARP * 6) + i];
+      h = s_bra + i / 6; r = i % 6;
+    } else {
+      const int ii = i - TDG_WARP * 6;
+#pragma unroll
+      for (int w = 0; w < TDG_WARPS; ++w) v += s_gk[w * (TDG_KB * 6) + ii];
+      h = s_ket + ii / 6; r = ii % 6;
     }
+    if (v != 0.0) red_add(P.grad + 3 * (r < 3 ? h->atomA : h->atomB) + (r < 3 ? r : r - 3), v);
   }
   // stats
   for (int o = 16; o > 0; o >>= 1) {
