@@ -111,6 +111,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(ms, dist, device):
+    """Timing rule for N > 1: the step time is the MAX over ranks (replicas run independently, no data-path collective)."""
+    if dist is None:
+        return float(ms)
+    import torch
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, quartets_per_rank, ms):
+    """Whole-job throughput: every rank processed `quartets_per_rank` quartets in `ms` (max over ranks)."""
+    return world * quartets_per_rank / (ms * 1e-3)
+
+
 def run_ours(args):
     import torch
 
@@ -166,13 +182,10 @@ def run_ours(args):
     barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if sampler else None
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, dev)
     g_host = g_dev.cpu().numpy()
     if rank == 0:
-        value = world * quartets / (ms * 1e-3)
+        value = aggregate_value(world, quartets, ms)
         # roofline of the dominant class kernel (largest share of the step)
         top = max(range(tdgrad.NCLASS), key=lambda c: agg_ms[c])
         fl_top = tdgrad.model_flops(top, agg_q[top], agg_p[top])

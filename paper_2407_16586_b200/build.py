@@ -15,10 +15,11 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libtdgrad.so")
 LMAX = 3
 PAIR_CLASSES = [(la, lb) for la in range(LMAX + 1) for lb in range(la + 1)]
+QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASSES[: i + 1]]   # bra class >= ket class
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-DTDG_LMAX_BUILD=%d" % LMAX]
-HEADERS = ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "../../include/tdgrad.h"]
+HEADERS = ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "rys_tables.inc", "../../include/tdgrad.h"]
 
 
 def _newest_header() -> float:
@@ -37,8 +38,11 @@ def _compile(job):
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     jobs = [("tdg_api.cu", os.path.join(OBJ, "tdg_api.o"), []), ("tdg_aux.cu", os.path.join(OBJ, "tdg_aux.o"), [])]
-    for la, lb in PAIR_CLASSES:
-        jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d.o" % (la, lb)), ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb]))
+    for la, lb, lc, ld in QUARTET_CLASSES:
+        jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d%d%d.o" % (la, lb, lc, ld)),
+                     ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb, "-DTDG_LC=%d" % lc, "-DTDG_LD=%d" % ld]))
+    # longest compiles first (fully unrolled d-shell classes)
+    jobs.sort(key=lambda j: 0 if "class" not in j[1] else -sum(int(c) for c in os.path.basename(j[1])[10:14]))
     hdr = _newest_header()
     todo = []
     for src, obj, extra in jobs:

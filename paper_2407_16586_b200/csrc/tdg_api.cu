@@ -14,34 +14,15 @@
 
 #define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
 
-tdg_launch_fn tdg_class_launcher_00(int, int);
-tdg_launch_fn tdg_class_launcher_10(int, int);
-tdg_launch_fn tdg_class_launcher_11(int, int);
-tdg_launch_fn tdg_class_launcher_20(int, int);
-tdg_launch_fn tdg_class_launcher_21(int, int);
-tdg_launch_fn tdg_class_launcher_22(int, int);
-#if TDG_LMAX_BUILD >= 3
-tdg_launch_fn tdg_class_launcher_30(int, int);
-tdg_launch_fn tdg_class_launcher_31(int, int);
-tdg_launch_fn tdg_class_launcher_32(int, int);
-tdg_launch_fn tdg_class_launcher_33(int, int);
-#endif
+#define TDG_CLASS(la, lb, lc, ld) tdg_launch_fn tdg_class_launcher_##la##lb##lc##ld();
+#include "tdg_classes.inc"
+#undef TDG_CLASS
 
 tdg_launch_fn tdg_get_launcher(int la, int lb, int lc, int ld) {
-  switch (PCLS(la, lb)) {
-    case 0: return tdg_class_launcher_00(lc, ld);
-    case 1: return tdg_class_launcher_10(lc, ld);
-    case 2: return tdg_class_launcher_11(lc, ld);
-    case 3: return tdg_class_launcher_20(lc, ld);
-    case 4: return tdg_class_launcher_21(lc, ld);
-    case 5: return tdg_class_launcher_22(lc, ld);
-#if TDG_LMAX_BUILD >= 3
-    case 6: return tdg_class_launcher_30(lc, ld);
-    case 7: return tdg_class_launcher_31(lc, ld);
-    case 8: return tdg_class_launcher_32(lc, ld);
-    case 9: return tdg_class_launcher_33(lc, ld);
-#endif
-  }
+#define TDG_CLASS(a, b, c, d) \
+  if (la == a && lb == b && lc == c && ld == d) return (a <= TDG_LMAX_BUILD) ? tdg_class_launcher_##a##b##c##d() : nullptr;
+#include "tdg_classes.inc"
+#undef TDG_CLASS
   return nullptr;
 }
 

@@ -1,42 +1,21 @@
-// tdg_class.cu — instantiates the gradient kernels of one bra pair class (compile with -DTDG_LA=.. -DTDG_LB=..);
-// one kernel per non-redundant angular class: ket pair class <= bra pair class.
+// tdg_class.cu — instantiates the gradient kernel of ONE quartet class; compile with
+// -DTDG_LA=.. -DTDG_LB=.. -DTDG_LC=.. -DTDG_LD=.. (one kernel per non-redundant angular class).
 #include "tdg_grad.cuh"
 
-#ifndef TDG_LA
-#error "compile with -DTDG_LA=<la> -DTDG_LB=<lb>"
+#if !defined(TDG_LA) || !defined(TDG_LB) || !defined(TDG_LC) || !defined(TDG_LD)
+#error "compile with -DTDG_LA=<la> -DTDG_LB=<lb> -DTDG_LC=<lc> -DTDG_LD=<ld>"
 #endif
-#define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
 
-template <int LC, int LD>
 static void launch(const KParams& P, int nblocks, cudaStream_t s) {
-  typedef QC<TDG_LA, TDG_LB, LC, LD> C;
+  typedef QC<TDG_LA, TDG_LB, TDG_LC, TDG_LD> C;
   constexpr int smem = (C::RYS_SH_DOUBLES + TDG_ACC_DOUBLES) * (int)sizeof(double);
   static bool attr_set = false;
-  if (!attr_set && smem > 0) {
-    cudaFuncSetAttribute(tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (!attr_set) {
+    cudaFuncSetAttribute(tdg_grad_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     attr_set = true;
   }
-  tdg_grad_kernel<TDG_LA, TDG_LB, LC, LD><<<dim3(nblocks, C::NROLE), TDG_WARPS * TDG_WARP, smem, s>>>(P);
+  tdg_grad_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD><<<dim3(nblocks, C::NROLE), TDG_WARPS * TDG_WARP, smem, s>>>(P);
 }
-template <int LC, int LD>
-static tdg_launch_fn pick() {
-  if constexpr (PCLS(LC, LD) <= PCLS(TDG_LA, TDG_LB) && LC <= TDG_LMAX_BUILD) return &launch<LC, LD>;
-  else return nullptr;
-}
-#define TDG_CAT2(a, b, c) a##b##c
-#define TDG_CAT(a, b, c) TDG_CAT2(a, b, c)
-tdg_launch_fn TDG_CAT(tdg_class_launcher_, TDG_LA, TDG_LB)(int lc, int ld) {
-  switch (PCLS(lc, ld)) {
-    case 0: return pick<0, 0>();
-    case 1: return pick<1, 0>();
-    case 2: return pick<1, 1>();
-    case 3: return pick<2, 0>();
-    case 4: return pick<2, 1>();
-    case 5: return pick<2, 2>();
-    case 6: return pick<3, 0>();
-    case 7: return pick<3, 1>();
-    case 8: return pick<3, 2>();
-    case 9: return pick<3, 3>();
-  }
-  return nullptr;
-}
+#define TDG_CAT2(a, b, c, d, e) a##b##c##d##e
+#define TDG_CAT(a, b, c, d, e) TDG_CAT2(a, b, c, d, e)
+tdg_launch_fn TDG_CAT(tdg_class_launcher_, TDG_LA, TDG_LB, TDG_LC, TDG_LD)() { return &launch; }

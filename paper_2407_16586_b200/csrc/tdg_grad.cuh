@@ -20,7 +20,7 @@
 #define TDG_RU_LIM 120
 #endif
 #ifndef TDG_MAX_ROLES
-#define TDG_MAX_ROLES 6   // classes needing more roles keep rolled loops (compile time)
+#define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dp), (dd|dd), f shells) keep rolled loops (compile time)
 #endif
 
 template <int LA, int LB, int LC, int LD>

@@ -1,0 +1,45 @@
+"""N > 1 path of bench.py on CPU: two gloo ranks, max-over-ranks timing and whole-job aggregation (replicas only:
+the path has no data-path collective this round)."""
+import os
+import sys
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    import bench
+
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = bench.max_over_ranks(100.0 + 50.0 * rank, dist, torch.device("cpu"))
+    dist.barrier()
+    if rank == 0:
+        out.put((ms, bench.aggregate_value(world, 1000, ms)))
+    dist.destroy_process_group()
+
+
+def test_two_rank_timing_and_aggregation():
+    ctx = mp.get_context("spawn")
+    q = ctx.SimpleQueue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    ms, value = q.get()
+    assert ms == 150.0
+    assert abs(value - 2 * 1000 / 0.150) < 1e-9
+
+
+def test_single_rank_passthrough():
+    sys.path.insert(0, ROOT)
+    import bench
+
+    assert bench.max_over_ranks(12.5, None, None) == 12.5
