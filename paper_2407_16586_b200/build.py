@@ -19,7 +19,7 @@ QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASS
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-DTDG_LMAX_BUILD=%d" % LMAX]
-HEADERS = ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "rys_tables.inc", "../../include/tdgrad.h"]
+HEADERS = ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc", "../../include/tdgrad.h"]
 
 
 def _newest_header() -> float:

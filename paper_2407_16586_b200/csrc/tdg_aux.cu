@@ -3,11 +3,19 @@
 #include "tdg_common.cuh"
 #include "tdg_internal.h"
 #include "rys_tables.inc"
+#undef BOYS_PER_UNIT
+#undef BOYS_K
+#include "boys_tables.inc"
 
+// device table = [Rys polynomial tables | Boys Taylor tables] (rys_part_off)
 cudaError_t tdg_upload_rys_table(double** d_tab) {
-  cudaError_t e = cudaMalloc(d_tab, sizeof(RYS_TAB));
+  static_assert(sizeof(RYS_TAB) / sizeof(double) == rys_off(RYS_NMAX + 1), "table size");
+  static_assert(sizeof(BOYS_TAB) / sizeof(double) == rys_part_off(2) - rys_part_off(1) + rys_part_doubles(2), "boys table size");
+  cudaError_t e = cudaMalloc(d_tab, sizeof(RYS_TAB) + sizeof(BOYS_TAB));
   if (e != cudaSuccess) return e;
-  return cudaMemcpy(*d_tab, RYS_TAB, sizeof(RYS_TAB), cudaMemcpyHostToDevice);
+  e = cudaMemcpy(*d_tab, RYS_TAB, sizeof(RYS_TAB), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*d_tab + sizeof(RYS_TAB) / sizeof(double), BOYS_TAB, sizeof(BOYS_TAB), cudaMemcpyHostToDevice);
 }
 
 // ---------------------------------------------------------------------------------------------------------

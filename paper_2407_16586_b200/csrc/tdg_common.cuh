@@ -128,9 +128,51 @@ __device__ __forceinline__ void rys_roots_tab(const double* __restrict__ tabN, d
     w[r] = ((N + r) & 1) ? v[(N + r) >> 1].y : v[(N + r) >> 1].x;
   }
 }
+// n <= 2: closed-form rule from the Boys moments F_0..F_{2n-1} (fewer table loads than the polynomial tables: one
+// 64-byte Taylor row for F_{2n-1}, downward recursion F_{m-1} = (2T F_m + e^-T)/(2m-1), then x = F1/F0, w = F0 for n = 1
+// and the roots of the monic orthogonal quadratic of the 2x2 Hankel system for n = 2).  boys_tables.inc layout.
+#define BOYS_PER_UNIT 8
+#define BOYS_K 8
+template <int N>
+__device__ __forceinline__ void rys_roots_boys(const double* __restrict__ tabN, double T, double* __restrict__ x, double* __restrict__ w) {
+  static_assert(N == 1 || N == 2, "closed form only for n <= 2");
+  if (T >= (double)rys_tmax(N)) {
+    double rT = 1.0 / T, rs = sqrt(rT);
+#pragma unroll
+    for (int r = 0; r < N; ++r) { x[r] = rys_inf(N, r) * rT; w[r] = rys_inf(N, N + r) * rs; }
+    return;
+  }
+  const int i = (int)(T * BOYS_PER_UNIT);
+  const double d = T - ((double)i + 0.5) * (1.0 / BOYS_PER_UNIT);
+  const double2* c = reinterpret_cast<const double2*>(tabN + i * BOYS_K);
+  const double2 c01 = c[0], c23 = c[1], c45 = c[2], c67 = c[3];
+  double F = fma(c67.y, d, c67.x);
+  F = fma(F, d, c45.y); F = fma(F, d, c45.x); F = fma(F, d, c23.y); F = fma(F, d, c23.x); F = fma(F, d, c01.y); F = fma(F, d, c01.x);
+  const double e = exp(-T), T2 = 2.0 * T;
+  if (N == 1) {
+    const double F0 = fma(T2, F, e);
+    x[0] = F / F0; w[0] = F0;
+  } else {
+    const double m3 = F, m2 = fma(T2, m3, e) * 0.2, m1 = fma(T2, m2, e) * (1.0 / 3.0), m0 = fma(T2, m1, e);
+    const double rdet = 1.0 / (m0 * m2 - m1 * m1);
+    const double c1 = (m1 * m2 - m0 * m3) * rdet, c0 = (m1 * m3 - m2 * m2) * rdet;
+    const double x2 = 0.5 * (sqrt(c1 * c1 - 4.0 * c0) - c1), x1 = c0 / x2;
+    const double w1 = (m0 * x2 - m1) / (x2 - x1);
+    x[0] = x1; x[N - 1] = x2; w[0] = w1; w[N - 1] = m0 - w1;
+  }
+}
+// Device table = [Rys polynomial tables | Boys Taylor tables]; offset/size of the part a class with N roots uses.
+__host__ __device__ constexpr int rys_part_off(int n) { return n <= 2 ? rys_off(RYS_NMAX + 1) + (n == 2 ? rys_tmax(1) * BOYS_PER_UNIT * BOYS_K : 0) : rys_off(n); }
+__host__ __device__ constexpr int rys_part_doubles(int n) { return n <= 2 ? rys_tmax(n) * BOYS_PER_UNIT * BOYS_K : RYS_TABLE_DOUBLES(n); }
+// `part` points at rys_part_off(N) of the device table (or at a shared-memory copy of that part)
+template <int N>
+__device__ __forceinline__ void rys_eval(const double* __restrict__ part, double T, double* __restrict__ x, double* __restrict__ w) {
+  if constexpr (N <= 2) rys_roots_boys<N>(part, T, x, w);
+  else rys_roots_tab<N>(part, T, x, w);
+}
 template <int N>
 __device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double T, double* __restrict__ x, double* __restrict__ w) {
-  rys_roots_tab<N>(tab + rys_off(N), T, x, w);
+  rys_eval<N>(tab + rys_part_off(N), T, x, w);
 }
 
 __device__ __forceinline__ double warp_sum(double v) {

@@ -43,7 +43,7 @@ struct QC {
   static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;
   static constexpr bool RYS_SH = NR <= 4;                                  // Rys table of this NR staged in shared memory
-  static constexpr int RYS_SH_DOUBLES = RYS_SH ? RYS_TABLE_DOUBLES(NR) : 0;
+  static constexpr int RYS_SH_DOUBLES = RYS_SH ? rys_part_doubles(NR) : 0;
   static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
 };
 
@@ -197,7 +197,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
         double s2 = 1.0, ss = 1.0;
         if (op == 1) { s2 = P.omega2 / (P.omega2 + rho); ss = sqrt(s2); }
         double xr[NR], wr[NR];
-        rys_roots_tab<NR>(rys, s2 * T, xr, wr);
+        rys_eval<NR>(rys, s2 * T, xr, wr);
         const double* __restrict__ G = op == 0 ? GF : GL;
 #pragma unroll(RU)
         for (int r = 0; r < NR; ++r) {
@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
   if (ket_ok) s_ket[t] = P.ket_hdr[k];
   for (int i = t; i < TDG_WARPS * TDG_WARP * 6; i += TDG_NT) s_gb[i] = 0.0;
   for (int i = t; i < TDG_WARPS * TDG_KB * 6; i += TDG_NT) s_gk[i] = 0.0;
-  const double* rys = P.rys_tab + rys_off(C::NR);
+  const double* rys = P.rys_tab + rys_part_off(C::NR);
   if (C::RYS_SH) {
     const double2* src = reinterpret_cast<const double2*>(rys);
     for (int i = t; i < C::RYS_SH_DOUBLES / 2; i += TDG_NT) s_rys[i] = __ldg(src + i);
