@@ -28,7 +28,7 @@ def _newest_header() -> float:
 
 def _compile(job):
     src, obj, extra = job
-    cmd = [NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
+    cmd = [NVCC] + FLAGS + os.environ.get("TDG_EXTRA_FLAGS", "").split() + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
@@ -49,6 +49,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         st = max(os.path.getmtime(os.path.join(CSRC, src)), hdr, os.path.getmtime(os.path.abspath(__file__)))
         if force or not os.path.exists(obj) or os.path.getmtime(obj) < st:
             todo.append((src, obj, extra))
+    only = os.environ.get("TDG_ONLY")   # developer aid: recompile only these classes (e.g. "1000,1110"), reuse the other objects
+    if only:
+        keep = tuple("tdg_class_%s.o" % c for c in only.split(","))
+        todo = [j for j in jobs if j[1].endswith(keep) or not os.path.exists(j[1])]
     if todo:
         if verbose:
             print("compiling %d objects" % len(todo), file=sys.stderr)

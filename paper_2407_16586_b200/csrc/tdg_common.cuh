@@ -175,6 +175,15 @@ __device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double
   rys_eval<N>(tab + rys_part_off(N), T, x, w);
 }
 
+// 256-bit read-only global load (sm_100: LDG.E.256): 4 doubles from a 32-byte-aligned address in ONE load instruction;
+// the density gathers and primitive-pair records are lane-divergent, so the L1 cost is per instruction, not per byte.
+struct d4 { double x, y, z, w; };
+__device__ __forceinline__ d4 ld256(const double* p) {
+  d4 v;
+  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -19,6 +19,9 @@
 #ifndef TDG_RU_LIM
 #define TDG_RU_LIM 120
 #endif
+#ifndef TDG_ROLE_COMPS
+#define TDG_ROLE_COMPS 27   // target number of function quartets per role
+#endif
 #ifndef TDG_MAX_ROLES
 #define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dp), (dd|dd), f shells) keep rolled loops (compile time)
 #endif
@@ -36,12 +39,13 @@ struct QC {
   // registers; the 2-D integrals are rebuilt by every role.  Classes with an f shell keep rolled loops (one role).
   static constexpr bool HASF = LA == 3 || LB == 3 || LC == 3 || LD == 3;
   static constexpr int NAB = NA * NB, KDN = NC * ND;
-  static constexpr int ABN1 = 27 / KDN >= NAB ? NAB : (27 / KDN > 0 ? 27 / KDN : 1);
+  static constexpr int ABN1 = TDG_ROLE_COMPS / KDN >= NAB ? NAB : (TDG_ROLE_COMPS / KDN > 0 ? TDG_ROLE_COMPS / KDN : 1);
   static constexpr int NROLE1 = (NAB + ABN1 - 1) / ABN1;
   static constexpr bool SMALL = NCOMP <= 27 || (!HASF && NROLE1 <= TDG_MAX_ROLES);   // fully unrolled code
   static constexpr int NROLE = SMALL ? NROLE1 : 1;
   static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;
+  static constexpr bool PREFETCH = false;   // software prefetch of the next quartet's blocks: measured SLOWER (L1 wavefront-bound), kept off
   static constexpr bool RYS_SH = NR <= 4;                                  // Rys table of this NR staged in shared memory
   static constexpr int RYS_SH_DOUBLES = RYS_SH ? rys_part_doubles(NR) : 0;
   static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
@@ -127,46 +131,46 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
     //   Gt_K = u.MK.v + s.MK.t,  u = pk(ik)[a,c], v = pk(jl)[b,d], s = pk(jk)[b,c], t = pk(il)[a,d];  Gt_J = pk(ij)[a,b].MJ.pk(kl)[c,d]
     const size_t n = (size_t)P.nbf;
     const double* __restrict__ pk = P.pk;
-    const double2* bIK = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offA * n + (size_t)NA * kh.offA));
-    const double2* bJL = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offB * n + (size_t)NB * kh.offB));
-    const double2* bJK = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offB * n + (size_t)NB * kh.offA));
-    const double2* bIL = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offA * n + (size_t)NA * kh.offB));
-    const double2* bIJ = reinterpret_cast<const double2*>(pk + 4 * ((size_t)bh.offA * n + (size_t)NA * bh.offB));
-    const double2* bKL = reinterpret_cast<const double2*>(pk + 4 * ((size_t)kh.offA * n + (size_t)NC * kh.offB));
+    const double* bIK = pk + 4 * ((size_t)bh.offA * n + (size_t)NA * kh.offA);
+    const double* bJL = pk + 4 * ((size_t)bh.offB * n + (size_t)NB * kh.offB);
+    const double* bJK = pk + 4 * ((size_t)bh.offB * n + (size_t)NB * kh.offA);
+    const double* bIL = pk + 4 * ((size_t)bh.offA * n + (size_t)NA * kh.offB);
+    const double* bIJ = pk + 4 * ((size_t)bh.offA * n + (size_t)NA * bh.offB);
+    const double* bKL = pk + 4 * ((size_t)kh.offA * n + (size_t)NC * kh.offB);
     // transformed small blocks: MK.v (jl), MK.t (il), MJ.(kl)
     double vJL[NB * ND][4], tIL[NA * ND][4], vKL[NC * ND][4];
 #pragma unroll(U)
     for (int e = 0; e < NB * ND; ++e) {
-      const double2 x0 = __ldg(bJL + 2 * e), x1 = __ldg(bJL + 2 * e + 1);
+      const d4 x = ld256(bJL + 4 * e);
 #pragma unroll
-      for (int m = 0; m < 4; ++m) vJL[e][m] = P.MK[4 * m] * x0.x + P.MK[4 * m + 1] * x0.y + P.MK[4 * m + 2] * x1.x + P.MK[4 * m + 3] * x1.y;
+      for (int m = 0; m < 4; ++m) vJL[e][m] = P.MK[4 * m] * x.x + P.MK[4 * m + 1] * x.y + P.MK[4 * m + 2] * x.z + P.MK[4 * m + 3] * x.w;
     }
 #pragma unroll(U)
     for (int e = 0; e < NA * ND; ++e) {
-      const double2 x0 = __ldg(bIL + 2 * e), x1 = __ldg(bIL + 2 * e + 1);
+      const d4 x = ld256(bIL + 4 * e);
 #pragma unroll
-      for (int m = 0; m < 4; ++m) tIL[e][m] = P.MK[4 * m] * x0.x + P.MK[4 * m + 1] * x0.y + P.MK[4 * m + 2] * x1.x + P.MK[4 * m + 3] * x1.y;
+      for (int m = 0; m < 4; ++m) tIL[e][m] = P.MK[4 * m] * x.x + P.MK[4 * m + 1] * x.y + P.MK[4 * m + 2] * x.z + P.MK[4 * m + 3] * x.w;
     }
 #pragma unroll(U)
     for (int e = 0; e < NC * ND; ++e) {
-      const double2 x0 = __ldg(bKL + 2 * e), x1 = __ldg(bKL + 2 * e + 1);
+      const d4 x = ld256(bKL + 4 * e);
 #pragma unroll
-      for (int m = 0; m < 4; ++m) vKL[e][m] = P.MJ[4 * m] * x0.x + P.MJ[4 * m + 1] * x0.y + P.MJ[4 * m + 2] * x1.x + P.MJ[4 * m + 3] * x1.y;
+      for (int m = 0; m < 4; ++m) vKL[e][m] = P.MJ[4 * m] * x.x + P.MJ[4 * m + 1] * x.y + P.MJ[4 * m + 2] * x.z + P.MJ[4 * m + 3] * x.w;
     }
 #pragma unroll(U)
     for (int ab = AB0; ab < AB0 + ABC; ++ab) {
       {
         const int a = ab / NB, b = ab - a * NB;
-        const double2 j0 = __ldg(bIJ + 2 * (a * NB + b)), j1 = __ldg(bIJ + 2 * (a * NB + b) + 1);
+        const d4 jv = ld256(bIJ + 4 * (a * NB + b));
 #pragma unroll(U)
         for (int c = 0; c < NC; ++c) {
-          const double2 u0 = __ldg(bIK + 2 * (a * NC + c)), u1 = __ldg(bIK + 2 * (a * NC + c) + 1);
-          const double2 s0 = __ldg(bJK + 2 * (b * NC + c)), s1 = __ldg(bJK + 2 * (b * NC + c) + 1);
+          const d4 u = ld256(bIK + 4 * (a * NC + c));
+          const d4 sv = ld256(bJK + 4 * (b * NC + c));
 #pragma unroll(U)
           for (int d = 0; d < ND; ++d) {
             const double* v = vJL[b * ND + d]; const double* tt = tIL[a * ND + d]; const double* w = vKL[c * ND + d];
-            const double gk = u0.x * v[0] + u0.y * v[1] + u1.x * v[2] + u1.y * v[3] + s0.x * tt[0] + s0.y * tt[1] + s1.x * tt[2] + s1.y * tt[3];
-            const double gj = j0.x * w[0] + j0.y * w[1] + j1.x * w[2] + j1.y * w[3];
+            const double gk = u.x * v[0] + u.y * v[1] + u.z * v[2] + u.w * v[3] + sv.x * tt[0] + sv.y * tt[1] + sv.z * tt[2] + sv.w * tt[3];
+            const double gj = jv.x * w[0] + jv.y * w[1] + jv.z * w[2] + jv.w * w[3];
             const double cn = deg * c_cnorm[LA][a] * c_cnorm[LB][b] * c_cnorm[LC][c] * c_cnorm[LD][d];
             const int idx = ((ab - AB0) * NC + c) * ND + d;
             GF[idx] = cn * (gj + P.cK * gk);
@@ -181,12 +185,12 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
   const double ABx = bh.AB[0], ABy = bh.AB[1], ABz = bh.AB[2];
   const double CDx = kh.AB[0], CDy = kh.AB[1], CDz = kh.AB[2];
   for (int ib = 0; ib < P.nppb; ++ib) {
-    const double* bp = bprim + ib * TDG_PRIM_STRIDE;
-    const double p = bp[0], Px = bp[1], Py = bp[2], Pz = bp[3], Kab = bp[4], a2 = 2.0 * bp[5], b2 = 2.0 * bp[6];
+    const d4 bp0 = ld256(bprim + ib * TDG_PRIM_STRIDE), bp1 = ld256(bprim + ib * TDG_PRIM_STRIDE + 4);
+    const double p = bp0.x, Px = bp0.y, Py = bp0.z, Pz = bp0.w, Kab = bp1.x, a2 = 2.0 * bp1.y, b2 = 2.0 * bp1.z;
     const double PAx = Px - bh.A[0], PAy = Py - bh.A[1], PAz = Pz - bh.A[2];
     for (int ik = 0; ik < P.nppk; ++ik) {
-      const double* kp = kprim + ik * TDG_PRIM_STRIDE;
-      const double q = __ldg(kp + 0), Qx = __ldg(kp + 1), Qy = __ldg(kp + 2), Qz = __ldg(kp + 3), Kcd = __ldg(kp + 4), c2 = 2.0 * __ldg(kp + 5);
+      const d4 kp0 = ld256(kprim + ik * TDG_PRIM_STRIDE), kp1 = ld256(kprim + ik * TDG_PRIM_STRIDE + 4);
+      const double q = kp0.x, Qx = kp0.y, Qy = kp0.z, Qz = kp0.w, Kcd = kp1.x, c2 = 2.0 * kp1.y;
       const double QCx = Qx - kh.A[0], QCy = Qy - kh.A[1], QCz = Qz - kh.A[2];
       const double PQx = Px - Qx, PQy = Py - Qy, PQz = Pz - Qz;
       const double rpq = 1.0 / (p + q), rho = p * q * rpq;
@@ -251,6 +255,27 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
 
 __device__ __forceinline__ void red_add(double* addr, double v) { atomicAdd(addr, v); }
 
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+// Prefetch the six packed density blocks and the primitive-pair data of the NEXT survivor of this lane into L1 while
+// the current quartet is computed (the density gathers are the long-scoreboard stalls of the low-l classes).
+template <int LA, int LB, int LC, int LD>
+__device__ __forceinline__ void prefetch_quartet(const KParams& P, const PairHdr& bh, const PairHdr& kh, const double* bprim, const double* kprim) {
+  typedef QC<LA, LB, LC, LD> C;
+  const size_t n = (size_t)P.nbf;
+  const char* pk = reinterpret_cast<const char*>(P.pk);
+  const char* blk[6] = {pk + 32 * ((size_t)bh.offA * n + (size_t)C::NA * kh.offA), pk + 32 * ((size_t)bh.offB * n + (size_t)C::NB * kh.offB),
+                        pk + 32 * ((size_t)bh.offB * n + (size_t)C::NB * kh.offA), pk + 32 * ((size_t)bh.offA * n + (size_t)C::NA * kh.offB),
+                        pk + 32 * ((size_t)bh.offA * n + (size_t)C::NA * bh.offB), pk + 32 * ((size_t)kh.offA * n + (size_t)C::NC * kh.offB)};
+  constexpr int bytes[6] = {C::NA * C::NC * 32, C::NB * C::ND * 32, C::NB * C::NC * 32, C::NA * C::ND * 32, C::NA * C::NB * 32, C::NC * C::ND * 32};
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+#pragma unroll
+    for (int o = 0; o < bytes[q]; o += 128) prefetch_l1(blk[q] + o);
+    if ((bytes[q] & 127) != 0 || bytes[q] > 128) prefetch_l1(blk[q] + bytes[q] - 32);   // last sector (blocks are only 32-byte aligned)
+  }
+  prefetch_l1(bprim); prefetch_l1(kprim);
+}
+
 // Phase 2 of the kernel for one role (slice [AB0, AB0+ABC) of the bra function pairs).
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
@@ -260,6 +285,7 @@ __device__ __forceinline__ void process_survivors(const KParams& P, const PairHd
   // both measured): lanes with the same ket are contiguous, so the ket-centre terms are summed by a segmented warp
   // shuffle scan and added by the segment head to this warp's private slot; the bra-centre terms are added to this
   // warp's private slots segment by segment (bras are distinct within a segment).  Fourth centre: eq 41.
+  typedef QC<LA, LB, LC, LD> C0;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double* my_gb = s_gb + warp * (TDG_WARP * 6);
   double* my_gk = s_gk + warp * (TDG_KB * 6);
@@ -268,6 +294,12 @@ __device__ __forceinline__ void process_survivors(const KParams& P, const PairHd
     const bool act = s < total;
     const unsigned e = act ? s_list[s] : 0u;
     const int kt = e >> 5, b = e & 31;
+    if (C0::PREFETCH && s + TDG_NT < total) {
+      const unsigned e2 = s_list[s + TDG_NT];
+      const int kt2 = e2 >> 5, b2 = e2 & 31;
+      prefetch_quartet<LA, LB, LC, LD>(P, s_bra[b2], s_ket[kt2], P.bra_prim + (size_t)(bra0 + b2) * P.nppb * TDG_PRIM_STRIDE,
+                                       P.ket_prim + (size_t)(k0 + kt2) * P.nppk * TDG_PRIM_STRIDE);
+    }
     double g[9];
     if (act) {
       const PairHdr& bh = s_bra[b];
