@@ -191,11 +191,17 @@ def run_ours(args):
         fl_top = tdgrad.model_flops(top, agg_q[top], agg_p[top])
         fl_all = sum(tdgrad.model_flops(c, agg_q[c], agg_p[c]) for c in range(tdgrad.NCLASS))
         achieved = fl_top / (agg_ms[top] * 1e-3) * 1e-12
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        traffic, executed = None, {}
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")   # numbers read off the committed ncu captures (data only)
         if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get(tdgrad.class_name(top))
-        roofline = dict(bound="alu", achieved=achieved, peak=peak_tf, unit="TFLOP/s", frac=achieved / peak_tf, traffic=traffic,
+            rec = json.load(open(tpath)).get(tdgrad.class_name(top))
+            if rec:
+                traffic = rec.get("dram_bytes")
+                executed = dict(executed_tflops=rec.get("executed_tflops"), executed_frac=rec.get("executed_tflops", 0.0) / peak_tf,
+                                fp64_pipe_pct=rec.get("fp64_pipe_pct"),
+                                executed_note="FP64 FLOPs actually executed (ncu: 2*DFMA+DMUL+DADD) by the largest launch of this kernel, "
+                                              "profiles/r01_ncu_full_*.md; `achieved` uses SURVEY.md 8(d)'s algorithmic model, which charges 2-4x more")
+        roofline = dict(bound="alu", achieved=achieved, peak=peak_tf, unit="TFLOP/s", frac=achieved / peak_tf, traffic=traffic, **executed,
                         kernel="tdg_grad_kernel" + tdgrad.class_name(top), kernel_share_of_step=agg_ms[top] / ms,
                         peak_source="FP64 FMA-chain microbenchmark run live on this GPU (tdg_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                         whole_step_model_tflops=fl_all / (ms * 1e-3) * 1e-12, whole_step_frac=fl_all / (ms * 1e-3) * 1e-12 / peak_tf)

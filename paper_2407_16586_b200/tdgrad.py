@@ -48,7 +48,12 @@ def lib():
     global _lib
     if _lib is None:
         if not os.path.exists(LIB_PATH):
-            raise TdgError("libtdgrad.so not built: run `python -m paper_2407_16586_b200.build` (there is no CPU fallback)")
+            try:   # build the CUDA library in-tree (nvcc, ~10 min); this is the product itself, not a fallback
+                from paper_2407_16586_b200 import build as _build
+
+                _build.build()
+            except Exception as exc:
+                raise TdgError("libtdgrad.so is missing and could not be built (%s); there is no CPU fallback" % exc)
         L = C.CDLL(LIB_PATH)
         L.tdg_strerror.restype = C.c_char_p
         L.tdg_last_error.restype = C.c_char_p
