@@ -100,7 +100,8 @@ int tdg_gradient(tdg_ctx* ctx, int npair, const double* const* A, const double* 
                  const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
                  void* stream, double* grad, int grad_on_device, tdg_stats* stats);
 
-/* Contracted energy E (same arguments; host result) for finite-difference checks; not tuned. */
+/* Contracted energy E (same arguments, same screening and subsample rule; HOST result; synchronises) for
+ * finite-difference checks of the gradient; runtime-l kernel, not tuned. */
 int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
                const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
                void* stream, double* E_host);

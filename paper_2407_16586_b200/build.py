@@ -19,11 +19,15 @@ QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASS
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-DTDG_LMAX_BUILD=%d" % LMAX]
-HEADERS = ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc", "../../include/tdgrad.h"]
+DEPS = {   # headers each source includes
+    "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "rys_meta.inc"],
+    "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
+    "tdg_api.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "../../include/tdgrad.h"],
+}
 
 
-def _newest_header() -> float:
-    return max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
+def _newest_header(src: str) -> float:
+    return max(os.path.getmtime(os.path.join(CSRC, h)) for h in DEPS[src])
 
 
 def _compile(job):
@@ -43,10 +47,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
                      ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb, "-DTDG_LC=%d" % lc, "-DTDG_LD=%d" % ld]))
     # longest compiles first (fully unrolled d-shell classes)
     jobs.sort(key=lambda j: 0 if "class" not in j[1] else -sum(int(c) for c in os.path.basename(j[1])[10:14]))
-    hdr = _newest_header()
     todo = []
     for src, obj, extra in jobs:
-        st = max(os.path.getmtime(os.path.join(CSRC, src)), hdr, os.path.getmtime(os.path.abspath(__file__)))
+        st = max(os.path.getmtime(os.path.join(CSRC, src)), _newest_header(src))
         if force or not os.path.exists(obj) or os.path.getmtime(obj) < st:
             todo.append((src, obj, extra))
     only = os.environ.get("TDG_ONLY")   # developer aid: recompile only these classes (e.g. "1000,1110"), reuse the other objects

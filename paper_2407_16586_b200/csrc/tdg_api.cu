@@ -335,7 +335,7 @@ struct Group { std::vector<int> pairs; std::vector<int> canon; };   // canonical
 
 static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int on_dev,
                            const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
-                           cudaStream_t st, tdg_stats* stats) {
+                           cudaStream_t st, tdg_stats* stats, double* E_host = nullptr) {
   const int n = ctx->nbf;
   const size_t mbytes = sizeof(double) * (size_t)n * n;
   std::fill(ctx->scratch_used.begin(), ctx->scratch_used.end(), false);
@@ -405,6 +405,12 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
     P.dmax = ctx->d_dmax;
     aux_launches += 2;
   }
+  double* d_E = nullptr;
+  if (E_host) {   // energy mode (tdg_energy): same screening and work lists, undifferentiated integrals
+    d_E = (double*)scratch_get(ctx, 264);
+    if (!d_E) return TDG_ENOMEM;
+    CK(cudaMemsetAsync(d_E, 0, sizeof(double), st));
+  }
   double* pk = (double*)scratch_get(ctx, 4 * mbytes);
   if (!pk) { ctx->err = "device allocation of the packed density array failed"; return TDG_ENOMEM; }
   P.pk = pk;
@@ -438,17 +444,22 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
       const Work& W = ctx->work[w];
       const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
       tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb);
-      if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+      if (!fn && !d_E) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
       P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
       P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
       P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
       P.counters = ctx->d_counters + 3 * (gi == 0 ? w : nw);   // quartet counts come from the first group only
       if (stats) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); evs.push_back(e); ev_cls.push_back(W.cls); }
-      fn(P, W.nblocks, st);
+      if (d_E) CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, st));
+      else fn(P, W.nblocks, st);
       ++launches;
     }
   }
   CK(cudaGetLastError());
+  if (d_E) {
+    CK(cudaMemcpyAsync(E_host, d_E, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+  }
   if (stats) {
     cudaEventRecord(ev2, st);
     CK(cudaStreamSynchronize(st));
@@ -494,11 +505,16 @@ extern "C" int tdg_gradient(tdg_ctx* ctx, int npair, const double* const* A, con
   return TDG_OK;
 }
 
-extern "C" int tdg_energy(tdg_ctx* ctx, int, const double* const*, const double* const*, int, const double*, const double*,
-                          double, double, double, double, void*, double*) {
+extern "C" int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
+                          const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
+                          void* stream, double* E_host) {
   if (!ctx) return TDG_EINVAL;
-  ctx->err = "tdg_energy: not built in this round";
-  return TDG_EUNSUPPORTED;
+  if (!A || !B || !wJ || !wK || !E_host || npair <= 0 || npair > TDG_MAXP) return TDG_EINVAL;
+  for (int k = 0; k < npair; ++k) if (!A[k] || !B[k]) return TDG_EINVAL;
+  if (cLR != 0.0 && !(omega > 0.0)) return TDG_EINVAL;
+  if (!ctx->planned) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  return run_contraction(ctx, npair, A, B, matrices_on_device, wJ, wK, cJ, cK, cLR, omega, (cudaStream_t)stream, nullptr, E_host);
 }
 
 extern "C" int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out) {

@@ -149,6 +149,127 @@ cudaError_t tdg_launch_schwarz(const DevShell* sh, int ns, const double* xyz, co
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Contracted energy E (eq (E) of include/tdgrad.h) for finite-difference checks: plain ERIs with n = floor(L/2)+1 roots,
+// density products recomputed from the packed blocks for every (function quartet, root).  Not tuned.
+__device__ static double quartet_energy(const KParams& P, int la, int lb, int lc, int ld, const PairHdr& bh,
+                                        const double* __restrict__ bprim, const PairHdr& kh, const double* __restrict__ kprim) {
+  const int na = ncart(la), nb = ncart(lb), nc = ncart(lc), nd = ncart(ld);
+  const int nr = (la + lb + lc + ld) / 2 + 1;
+  const size_t n = (size_t)P.nbf;
+  const double* pk = P.pk;
+  const double* bIK = pk + 4 * ((size_t)bh.offA * n + (size_t)na * kh.offA);
+  const double* bJL = pk + 4 * ((size_t)bh.offB * n + (size_t)nb * kh.offB);
+  const double* bJK = pk + 4 * ((size_t)bh.offB * n + (size_t)nb * kh.offA);
+  const double* bIL = pk + 4 * ((size_t)bh.offA * n + (size_t)na * kh.offB);
+  const double* bIJ = pk + 4 * ((size_t)bh.offA * n + (size_t)na * bh.offB);
+  const double* bKL = pk + 4 * ((size_t)kh.offA * n + (size_t)nc * kh.offB);
+  double Ix[256], Iy[256], Iz[256];
+  double e = 0.0;
+  for (int ib = 0; ib < P.nppb; ++ib) {
+    const double* bp = bprim + ib * TDG_PRIM_STRIDE;
+    const double p = bp[0], Px = bp[1], Py = bp[2], Pz = bp[3], Kab = bp[4];
+    for (int ik = 0; ik < P.nppk; ++ik) {
+      const double* kp = kprim + ik * TDG_PRIM_STRIDE;
+      const double q = kp[0], Qx = kp[1], Qy = kp[2], Qz = kp[3], Kcd = kp[4];
+      const double PQx = Px - Qx, PQy = Py - Qy, PQz = Pz - Qz;
+      const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+      const double T = rho * (PQx * PQx + PQy * PQy + PQz * PQz);
+      const double pref = 34.986836655249725693 * Kab * Kcd * rpq * sqrt(rpq) / rho;
+      for (int op = 0; op <= P.use_lr; ++op) {
+        double s2 = 1.0, ss = 1.0;
+        if (op == 1) { s2 = P.omega2 / (P.omega2 + rho); ss = sqrt(s2); }
+        double xr[7], wr[7];
+        rys_roots_rt(nr, P.rys_tab, s2 * T, xr, wr);
+        for (int r = 0; r < nr; ++r) {
+          const double x = xr[r] * s2, w = wr[r] * ss * pref;
+          const double b00 = 0.5 * x * rpq, b10 = (0.5 - q * b00) / p, b01 = (0.5 - p * b00) / q;
+          const double fq = q * rpq * x, fp = p * rpq * x;
+          build2d_rt(la, lb, lc, ld, (Px - bh.A[0]) - fq * PQx, (Qx - kh.A[0]) + fp * PQx, b00, b10, b01, bh.AB[0], kh.AB[0], 1.0, Ix);
+          build2d_rt(la, lb, lc, ld, (Py - bh.A[1]) - fq * PQy, (Qy - kh.A[1]) + fp * PQy, b00, b10, b01, bh.AB[1], kh.AB[1], 1.0, Iy);
+          build2d_rt(la, lb, lc, ld, (Pz - bh.A[2]) - fq * PQz, (Qz - kh.A[2]) + fp * PQz, b00, b10, b01, bh.AB[2], kh.AB[2], w, Iz);
+          for (int a = 0; a < na; ++a) {
+            const unsigned va = c_cart[la][a];
+            for (int b = 0; b < nb; ++b) {
+              const unsigned vb = c_cart[lb][b];
+              const double* jv = bIJ + 4 * (a * nb + b);
+              for (int c = 0; c < nc; ++c) {
+                const unsigned vc = c_cart[lc][c];
+                const double* u = bIK + 4 * (a * nc + c);
+                const double* sv = bJK + 4 * (b * nc + c);
+                for (int d = 0; d < nd; ++d) {
+                  const unsigned vd = c_cart[ld][d];
+                  const double* v = bJL + 4 * (b * nd + d);
+                  const double* tt = bIL + 4 * (a * nd + d);
+                  const double* wv = bKL + 4 * (c * nd + d);
+                  double gk = 0.0, gj = 0.0;
+                  for (int m = 0; m < 4; ++m)
+                    for (int m2 = 0; m2 < 4; ++m2) {
+                      gk += P.MK[4 * m + m2] * (u[m] * v[m2] + sv[m] * tt[m2]);
+                      gj += P.MJ[4 * m + m2] * jv[m] * wv[m2];
+                    }
+                  const double G = (op == 0 ? gj + P.cK * gk : P.cLR * gk) * c_cnorm[la][a] * c_cnorm[lb][b] * c_cnorm[lc][c] * c_cnorm[ld][d];
+                  const int ix = ((((va & 15) * 4 + (vb & 15)) * 4 + (vc & 15)) * 4 + (vd & 15));
+                  const int iy = (((((va >> 4) & 15) * 4 + ((vb >> 4) & 15)) * 4 + ((vc >> 4) & 15)) * 4 + ((vd >> 4) & 15));
+                  const int iz = (((((va >> 8) & 15) * 4 + ((vb >> 8) & 15)) * 4 + ((vc >> 8) & 15)) * 4 + ((vd >> 8) & 15));
+                  e += G * Ix[ix] * Iy[iy] * Iz[iz];
+                }
+              }
+            }
+          }
+        }
+      }
+    }
+  }
+  return e;
+}
+
+__global__ void __launch_bounds__(TDG_WARPS * TDG_WARP) energy_kernel(const __grid_constant__ KParams P, int la, int lb, int lc, int ld, double* E) {
+  const int item = blockIdx.x;
+  int lo = 0, hi = P.ntiles;
+  while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (P.cum[mid] <= item) lo = mid; else hi = mid; }
+  const int tile = lo, chunk = item - P.cum[tile];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int bra = tile * TDG_WARP + lane;
+  double e = 0.0;
+  if (bra < P.nbra) {
+    const PairHdr bh = P.bra_hdr[bra];
+    const int ns = P.nshell;
+    const int k0 = chunk * TDG_KB + warp * TDG_KW;
+    const int k1 = min(k0 + TDG_KW, P.nket);
+    for (int k = k0; k < k1; ++k) {
+      if (P.same_bucket && k > bra) break;
+      const PairHdr kh = P.ket_hdr[k];
+      if (P.tau > 0.0) {
+        const double qq = bh.Q * kh.Q;
+        if (!(qq >= P.tau)) continue;
+        if (P.density_weighted) {
+          const double dij = P.dmax[(size_t)bh.ish * ns + bh.jsh], dkl = P.dmax[(size_t)kh.ish * ns + kh.jsh];
+          const double dik = P.dmax[(size_t)bh.ish * ns + kh.ish], djl = P.dmax[(size_t)bh.jsh * ns + kh.jsh];
+          const double dil = P.dmax[(size_t)bh.ish * ns + kh.jsh], djk = P.dmax[(size_t)bh.jsh * ns + kh.ish];
+          const double x1 = dik * djl, x2 = dil * djk;
+          double W = P.CJ * dij * dkl; const double WK = P.CK * (x1 > x2 ? x1 : x2);
+          if (WK > W) W = WK;
+          if (qq * W < P.tau) continue;
+        }
+      }
+      if (!tdg_sample_keep(bh.ish, bh.jsh, kh.ish, kh.jsh, P.sample_mod, P.sample_seed)) continue;
+      double deg = 1.0;
+      if (bh.ish == bh.jsh) deg *= 0.5;
+      if (kh.ish == kh.jsh) deg *= 0.5;
+      if (P.same_bucket && k == bra) deg *= 0.5;
+      e += deg * quartet_energy(P, la, lb, lc, ld, bh, P.bra_prim + (size_t)bra * P.nppb * TDG_PRIM_STRIDE, kh,
+                                P.ket_prim + (size_t)k * P.nppk * TDG_PRIM_STRIDE);
+    }
+  }
+  e = warp_sum(e);
+  if (lane == 0 && e != 0.0) atomicAdd(E, e);
+}
+cudaError_t tdg_launch_energy(const KParams& P, int la, int lb, int lc, int ld, int nblocks, double* E, cudaStream_t s) {
+  energy_kernel<<<nblocks, TDG_WARPS * TDG_WARP, 0, s>>>(P, la, lb, lc, ld, E);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Density preparation (a3)
 __device__ __forceinline__ void atomic_max_nonneg(double* addr, double v) {
   atomicMax((unsigned long long*)addr, (unsigned long long)__double_as_longlong(v));

@@ -24,3 +24,8 @@ cudaError_t tdg_run_fp64_peak(double ms, double* tflops);
 // matrix (row-major, device) or nullptr (slot = 0); kind[m] = 0: symmetric part (M+M^T)/2, 1: antisymmetric part (M-M^T)/2.
 struct PackSrc { const double* src[4]; int kind[4]; };
 cudaError_t tdg_launch_pack(const PackSrc& ps, int n, const int* bf2sh, const DevShell* sh, double* pk, cudaStream_t s);
+
+// Contracted energy (tdg_energy): runtime-l, untuned; one launch per bucket pair, same work lists and screening as the
+// gradient kernels; *E (device) is accumulated with FP64 atomics.
+struct KParams;
+cudaError_t tdg_launch_energy(const KParams& P, int la, int lb, int lc, int ld, int nblocks, double* E, cudaStream_t s);

@@ -181,6 +181,21 @@ class Context:
         self._check(rc, "tdg_gradient")
         return g, (st.asdict() if st is not None else None)
 
+    def energy(self, pairs, wJ, wK, cJ, cK, cLR, omega, stream=None) -> float:
+        """Contracted energy E (host float) for the same arguments as :meth:`gradient` (untuned; for FD checks)."""
+        npair = len(pairs)
+        on_dev = 0 if isinstance(pairs[0][0], np.ndarray) else 1
+        keep = [(np.ascontiguousarray(a, dtype=np.float64), np.ascontiguousarray(b, dtype=np.float64)) for a, b in pairs] if not on_dev else list(pairs)
+        PA = (C.c_void_p * npair)(*[_ptr(a) for a, _ in keep])
+        PB = (C.c_void_p * npair)(*[_ptr(b) for _, b in keep])
+        wJ = np.ascontiguousarray(wJ, dtype=np.float64)
+        wK = np.ascontiguousarray(wK, dtype=np.float64)
+        e = C.c_double()
+        rc = lib().tdg_energy(self._h, C.c_int(npair), PA, PB, C.c_int(on_dev), C.c_void_p(wJ.ctypes.data), C.c_void_p(wK.ctypes.data),
+                              C.c_double(cJ), C.c_double(cK), C.c_double(cLR), C.c_double(omega), C.c_void_p(stream if stream else 0), C.byref(e))
+        self._check(rc, "tdg_energy")
+        return e.value
+
     def rys(self, n, T, rho=None, omega=0.0) -> np.ndarray:
         T = np.ascontiguousarray(T, dtype=np.float64)
         rho = np.ones_like(T) if rho is None else np.ascontiguousarray(rho, dtype=np.float64)

@@ -163,3 +163,50 @@ def test_cfg3_subsample_bench_configuration(ctx, orc):
     _compare(g, ref)
     assert st["pairs_kept"] == rst["pairs_kept"]
     assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 3
+
+
+@pytest.mark.parametrize("with_f", [False, True])
+def test_energy_vs_oracle(ctx, orc, with_f):
+    s = tiny_system(with_f=with_f)
+    D, P, T = densities(s.nbf)
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    ctx.set_system(s)
+    ctx.plan(0.0, 0)
+    e = ctx.energy(pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"])
+    ref, _ = orc.energy(s, pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"])
+    assert abs(e - ref) <= 1e-11 * max(1.0, abs(ref)), (e, ref)
+
+
+def test_energy_cfg1_screened(ctx, orc):
+    s = wl.make_system(1)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    ctx.set_system(s)
+    ctx.plan(s.tau, s.density_weighted)
+    e = ctx.energy(pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"])
+    ref, _ = orc.energy(s, pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"])
+    assert abs(e - ref) <= 1e-10 * abs(ref), (e, ref)
+
+
+def test_gpu_gradient_is_derivative_of_gpu_energy(ctx):
+    """Central finite differences of tdg_energy (h = 1e-4 bohr) against tdg_gradient, all on the GPU."""
+    import copy
+
+    s = tiny_system(with_f=False)
+    D, P, T = densities(s.nbf)
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    args = (pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"])
+    ctx.set_system(s)
+    ctx.plan(0.0, 0)
+    g, _ = ctx.gradient(*args)
+    h = 1e-4
+    for atom, x in ((0, 0), (1, 2), (2, 1)):
+        e = []
+        for sign in (+1, -1):
+            s2 = copy.deepcopy(s)
+            s2.xyz[atom, x] += sign * h
+            ctx.set_system(s2)
+            ctx.plan(0.0, 0)
+            e.append(ctx.energy(*args))
+        fd = (e[0] - e[1]) / (2 * h)
+        assert abs(fd - g[atom, x]) <= 1e-6, (atom, x, fd, g[atom, x])
