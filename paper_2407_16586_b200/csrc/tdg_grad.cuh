@@ -45,6 +45,7 @@ struct QC {
   static constexpr int NROLE = SMALL ? NROLE1 : 1;
   static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;
+  static constexpr bool TWO_STAGE = SMALL && NROLE <= 2;   // measured: faster for 1-2 roles, slower for classes with more roles
   static constexpr bool PREFETCH = false;   // software prefetch of the next quartet's blocks: measured SLOWER (L1 wavefront-bound), kept off
   static constexpr bool RYS_SH = NR <= 4;                                  // Rys table of this NR staged in shared memory
   static constexpr int RYS_SH_DOUBLES = RYS_SH ? rys_part_doubles(NR) : 0;
@@ -116,6 +117,19 @@ __device__ __forceinline__ void comp_exps(int idx, int& x, int& y, int& z) {
   else { unsigned v = c_cart[L][idx]; x = v & 15; y = (v >> 4) & 15; z = (v >> 8) & 15; }
 }
 
+// Compile-time mask of the bra exponent pairs (i, j) that occur, in any direction, among the function pairs
+// ab in [AB0, AB0+ABC) of a role: stage 2 of the contraction skips the others (their H entries are never touched).
+template <int LA, int LB, int AB0, int ABC>
+constexpr unsigned make_touch() {   // bit i*5+j
+  unsigned m = 0;
+  for (int ab = AB0; ab < AB0 + ABC; ++ab) {
+    const int a = ab / ncart(LB), b = ab - a * ncart(LB);
+    for (int d = 0; d < 3; ++d) m |= 1u << (cart_exp(LA, a, d) * 5 + cart_exp(LB, b, d));
+  }
+  return m;
+}
+template <int LA, int LB, int AB0, int ABC> struct Touch { static constexpr unsigned v = make_touch<LA, LB, AB0, ABC>(); };
+
 // Gradient contribution of one shell quartet: g[0..2] = d/dA, g[3..5] = d/dB, g[6..8] = d/dC (sum over all
 // functions, primitives, roots and both operators, already multiplied by deg and the density products).
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
@@ -125,6 +139,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
   typedef QC<LA, LB, LC, LD> C;
   constexpr int NA = C::NA, NB = C::NB, NC = C::NC, ND = C::ND, NR = C::NR, U = C::UNR, RU = C::RUNR;
   constexpr bool SM = C::SMALL;
+  typedef Touch<LA, LB, AB0, ABC> TM;
   // this role's bra function pairs: ab = a*NB + b in [AB0, AB0+ABC)
   double GF[ABC * NC * ND], GL[ABC * NC * ND];
   {  // step a7, part 1: symmetrised density products for every function quartet, from the packed blocks
@@ -212,6 +227,65 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
           build2d<LA, LB, LC, LD>(PAx - fq * PQx, QCx + fp * PQx, b00, b10, b01, ABx, CDx, 1.0, Ix);
           build2d<LA, LB, LC, LD>(PAy - fq * PQy, QCy + fp * PQy, b00, b10, b01, ABy, CDy, 1.0, Iy);
           build2d<LA, LB, LC, LD>(PAz - fq * PQz, QCz + fp * PQz, b00, b10, b01, ABz, CDz, w, Iz);
+          if constexpr (C::TWO_STAGE) {
+          // step a7, part 2, two stages.  Stage 1 sums the density products times the two undifferentiated directions
+          // over all functions that share the exponent tuple (i,j,k,l) of the third direction:
+          //   Hx[i,j,k,l] = sum_{functions with x-exponents (i,j,k,l)} Gt * Iy * Iz   (and cyclically Hy, Hz).
+          // Stage 2 applies the centre derivatives (eq 39/42) once per tuple instead of once per function quartet:
+          //   g_Ax += Hx[t] (2a Ix[i+1..] - i Ix[i-1..]),  g_Bx, g_Cx likewise.
+          double Hx[LA + 1][LB + 1][LC + 1][LD + 1], Hy[LA + 1][LB + 1][LC + 1][LD + 1], Hz[LA + 1][LB + 1][LC + 1][LD + 1];
+#pragma unroll(U)
+          for (int i = 0; i <= LA; ++i)
+#pragma unroll(U)
+            for (int j = 0; j <= LB; ++j)
+#pragma unroll(U)
+              for (int k = 0; k <= LC; ++k)
+#pragma unroll(U)
+                for (int l = 0; l <= LD; ++l) { Hx[i][j][k][l] = 0.0; Hy[i][j][k][l] = 0.0; Hz[i][j][k][l] = 0.0; }
+#pragma unroll(U)
+          for (int ab = AB0; ab < AB0 + ABC; ++ab) {
+            const int a = ab / NB, b = ab - a * NB;
+            int ax, ay, az; comp_exps<LA, SM>(a, ax, ay, az);
+            {
+              int bx, by, bz; comp_exps<LB, SM>(b, bx, by, bz);
+#pragma unroll(U)
+              for (int c = 0; c < NC; ++c) {
+                int cx, cy, cz; comp_exps<LC, SM>(c, cx, cy, cz);
+#pragma unroll(U)
+                for (int d = 0; d < ND; ++d) {
+                  int dx, dy, dz; comp_exps<LD, SM>(d, dx, dy, dz);
+                  const double Gv = G[((ab - AB0) * NC + c) * ND + d];
+                  const double X0 = Ix[ax][bx][cx][dx], Y0 = Iy[ay][by][cy][dy], Z0 = Iz[az][bz][cz][dz];
+                  const double gz = Gv * Z0;
+                  Hx[ax][bx][cx][dx] += gz * Y0;
+                  Hy[ay][by][cy][dy] += gz * X0;
+                  Hz[az][bz][cz][dz] += Gv * X0 * Y0;
+                }
+              }
+            }
+          }
+#pragma unroll(U)
+          for (int i = 0; i <= LA; ++i)
+#pragma unroll(U)
+            for (int j = 0; j <= LB; ++j) {
+              if (SM && !((TM::v >> (i * 5 + j)) & 1u)) continue;   // exponent pair (i,j) of the bra not present in this role's slice
+#pragma unroll(U)
+              for (int k = 0; k <= LC; ++k)
+#pragma unroll(U)
+                for (int l = 0; l <= LD; ++l) {
+                  const double hx = Hx[i][j][k][l], hy = Hy[i][j][k][l], hz = Hz[i][j][k][l];
+                  double dAx = a2 * Ix[i + 1][j][k][l], dAy = a2 * Iy[i + 1][j][k][l], dAz = a2 * Iz[i + 1][j][k][l];
+                  if (i > 0) { dAx -= i * Ix[i - 1][j][k][l]; dAy -= i * Iy[i - 1][j][k][l]; dAz -= i * Iz[i - 1][j][k][l]; }
+                  double dBx = b2 * Ix[i][j + 1][k][l], dBy = b2 * Iy[i][j + 1][k][l], dBz = b2 * Iz[i][j + 1][k][l];
+                  if (j > 0) { dBx -= j * Ix[i][j - 1][k][l]; dBy -= j * Iy[i][j - 1][k][l]; dBz -= j * Iz[i][j - 1][k][l]; }
+                  double dCx = c2 * Ix[i][j][k + 1][l], dCy = c2 * Iy[i][j][k + 1][l], dCz = c2 * Iz[i][j][k + 1][l];
+                  if (k > 0) { dCx -= k * Ix[i][j][k - 1][l]; dCy -= k * Iy[i][j][k - 1][l]; dCz -= k * Iz[i][j][k - 1][l]; }
+                  g[0] += hx * dAx; g[1] += hy * dAy; g[2] += hz * dAz;
+                  g[3] += hx * dBx; g[4] += hy * dBy; g[5] += hz * dBz;
+                  g[6] += hx * dCx; g[7] += hy * dCy; g[8] += hz * dCz;
+                }
+            }
+          } else {
           // step a7, part 2: contract the derivative integrals of this root with Gt
 #pragma unroll(U)
           for (int ab = AB0; ab < AB0 + ABC; ++ab) {
@@ -246,6 +320,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
                 }
               }
             }
+          }
           }
         }
       }
