@@ -3,6 +3,8 @@
 Tolerance (BASELINE.json north_star; reading S13): max|dg| <= 1e-9 E_h/bohr and max|dg|/max|g| <= 1e-10.
 Integer results (pair / quartet counts) must be identical.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -210,3 +212,19 @@ def test_gpu_gradient_is_derivative_of_gpu_energy(ctx):
             e.append(ctx.energy(*args))
         fd = (e[0] - e[1]) / (2 * h)
         assert abs(fd - g[atom, x]) <= 1e-6, (atom, x, fd, g[atom, x])
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("TDG_RUN_CFG4") != "1", reason="several minutes of CPU oracle time; set TDG_RUN_CFG4=1 (result of the round-1 run: profiles/r01_cfg4_parity.md)")
+def test_cfg4_subsample_largest_configuration(ctx, orc):
+    """1024 waters (25 600 bf, 21 GB packed densities): deterministic subsample both sides evaluate (S12)."""
+    s = wl.make_system(4)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(4))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, sample_mod=4000000, sample_seed=4)
+    d = float(np.max(np.abs(g - ref)))
+    print("cfg4 subsample: quartets gpu/oracle", st["quartets_computed"], rst["quartets_computed"], "pairs_kept", st["pairs_kept"], rst["pairs_kept"],
+          "max|dg|", d, "max|g|", float(np.max(np.abs(ref))))
+    _compare(g, ref)
+    assert st["pairs_kept"] == rst["pairs_kept"]
+    assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 3
