@@ -1,0 +1,50 @@
+"""CPU checks of the binding's host-side helpers (class indexing, the algorithmic FLOP model of DESIGN.md section 5) and of
+the workload generator's bookkeeping (sizes of BASELINE.json's configs)."""
+import numpy as np
+
+from paper_2407_16586_b200 import tdgrad
+from paper_2407_16586_b200 import workload as wl
+
+
+def test_class_index_roundtrip_and_names():
+    pcs = [(la, lb) for la in range(4) for lb in range(la + 1)]
+    seen = set()
+    for c1, (la, lb) in enumerate(pcs):
+        for c2, (lc, ld) in enumerate(pcs[: c1 + 1]):
+            cls = c1 * (c1 + 1) // 2 + c2
+            assert tdgrad.class_ls(cls) == (la, lb, lc, ld)
+            seen.add(cls)
+    assert seen == set(range(tdgrad.NCLASS))
+    assert tdgrad.class_name(0) == "(ss|ss)" and tdgrad.class_name(1) == "(ps|ss)" and tdgrad.class_name(54) == "(ff|ff)"
+    # 21 classes for l <= 2
+    assert sum(1 for c in range(55) if max(tdgrad.class_ls(c)) <= 2) == 21
+
+
+def test_flop_model_matches_survey_examples():
+    """SURVEY.md 8(d) quotes per-primitive-quartet examples: (ss|ss) ~0.5 k, (ps|ss) ~1.8 k, (pp|ps) ~11 k, (dd|dd) ~0.63 M."""
+    def per_prim(la, lb, lc, ld):
+        pcs = [(a, b) for a in range(4) for b in range(a + 1)]
+        c1, c2 = pcs.index((la, lb)), pcs.index((lc, ld))
+        return tdgrad.model_flops(c1 * (c1 + 1) // 2 + c2, 0, 1)
+    assert 400 < per_prim(0, 0, 0, 0) < 600
+    assert 1600 < per_prim(1, 0, 0, 0) < 2000
+    assert 9e3 < per_prim(1, 1, 1, 0) < 13e3
+    assert 5.5e5 < per_prim(2, 2, 2, 2) < 7e5
+    # linear in both unit counts
+    assert tdgrad.model_flops(1, 10, 40) == 10 * tdgrad.model_flops(1, 1, 0) + 40 * tdgrad.model_flops(1, 0, 1)
+
+
+def test_config_sizes_match_baseline_json():
+    expect = {0: (3, 12, 25), 1: (24, 96, 200), 2: (96, 416, 1120), 3: (768, 3072, 6400), 4: (3072, 12288, 25600)}
+    for cfg, (natom, nshell, nbf) in expect.items():
+        s = wl.make_system(cfg)
+        assert (s.natom, s.nshell, s.nbf) == (natom, nshell, nbf)
+    s0, s1 = wl.make_system(0), wl.make_system(1)
+    assert np.array_equal(s0.exps[: s0.shells[-1, 3] + s0.shells[-1, 2]], s1.exps[: s0.shells[-1, 3] + s0.shells[-1, 2]])  # one basis for all
+
+
+def test_default_call_weights():
+    D = np.eye(3); P = 2 * np.eye(3); T = np.ones((3, 3))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    assert [(a is D, b is D) for a, b in pairs[:1]] == [(True, True)] and pairs[1][1] is P and pairs[2][0] is T
+    assert list(wJ) == [2.0, 2.0, 2.0] and list(wK) == [1.0, 1.0, 1.0]
