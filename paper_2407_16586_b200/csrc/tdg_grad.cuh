@@ -489,13 +489,12 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
         const double qq = bh.Q * Qk;
         if (!(qq >= P.tau)) continue;
         ++n_vis;
-        if (dw) {
+        if (dw && qq * (P.CJ * s_dij[b] * dkl) < P.tau) {
+          // W = max(W_J, W_K) (S9): the J-type bound alone does not keep the quartet, so gather the four K-type maxima
           const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + ksh), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + lsh);
           const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + lsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + ksh);
           const double x1 = dik * djl, x2 = dil * djk;
-          double W = P.CJ * s_dij[b] * dkl; const double WK = P.CK * (x1 > x2 ? x1 : x2);
-          if (WK > W) W = WK;
-          if (qq * W < P.tau) continue;
+          if (qq * (P.CK * (x1 > x2 ? x1 : x2)) < P.tau) continue;
         }
       } else ++n_vis;
       if (!tdg_sample_keep(bh.ish, bh.jsh, ksh, lsh, P.sample_mod, P.sample_seed)) continue;
