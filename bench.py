@@ -146,6 +146,9 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     cfg = args.config
     ctx = tdgrad.Context(local)
+    shard = args.parallelism == "shard" and world > 1      # work items dealt over ranks + one all-reduce
+    if shard:
+        ctx.set_shard(rank, world)
     peak_tf = ctx.fp64_peak(400.0)
     sysm = wl.make_system(cfg)
     nbf, natom = sysm.nbf, sysm.natom
@@ -156,8 +159,13 @@ def run_ours(args):
     def step(mats, out, stats=True):
         ctx.set_system(sysm)                                   # a0
         ctx.plan(sysm.tau, sysm.density_weighted, 0, 0)       # a1-a2 (Schwarz on device, sort, work lists)
-        return ctx.gradient(mats, wJ, wK, wl.C_J, wl.C_K, wl.C_LR, wl.OMEGA, stream=torch.cuda.current_stream().cuda_stream,
-                            out=out, want_stats=stats)       # a3-a9
+        g, st = ctx.gradient(mats, wJ, wK, wl.C_J, wl.C_K, wl.C_LR, wl.OMEGA, stream=torch.cuda.current_stream().cuda_stream,
+                             out=out, want_stats=stats)      # a3-a9
+        if shard:                                              # the path's one exchange step: 3*natom doubles over NCCL
+            g = tdgrad.allreduce_partial(g if out is not None else torch.from_numpy(g).to(dev))
+            if out is None:
+                g = g.cpu().numpy()
+        return g, st
 
     def barrier():
         if dist is not None:
@@ -184,8 +192,32 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None
     ms = max_over_ranks(ms, dist, dev)
     g_host = g_dev.cpu().numpy()
+    total_quartets = quartets
+    if shard:   # every rank computed its own share of the quartets
+        tq = torch.tensor([quartets], dtype=torch.int64, device=dev)
+        dist.all_reduce(tq, op=dist.ReduceOp.SUM)
+        total_quartets = int(tq.item())
+    # end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region; rank 0 alone for replicas,
+    # every rank (partial gradients all-reduced, max over ranks) when the work is sharded
+    e2e_dt = None
+    if rank == 0 or shard:
+        hD, hP, hT = [x.cpu().pin_memory().numpy() for x in (D, P, T)]
+        hpairs, _, _ = wl.default_call(hD, hP, hT)
+        e2e_warm = 0 if ms / args.steps > 20000 else 1
+        for _ in range(e2e_warm):
+            step(hpairs, None, stats=False)
+        if shard:
+            barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        g2, _ = step(hpairs, None, stats=False)
+        torch.cuda.synchronize()
+        e2e_dt = time.perf_counter() - t0
+        if shard:
+            e2e_dt = max_over_ranks(e2e_dt, dist, dev)
+        assert np.max(np.abs(g2 - g_host)) < 1e-8, "host-buffer and device-buffer paths disagree"
     if rank == 0:
-        value = aggregate_value(world, quartets, ms)
+        value = aggregate_value(1, total_quartets, ms) if shard else aggregate_value(world, quartets, ms)
         # roofline of the dominant class kernel (largest share of the step)
         top = max(range(tdgrad.NCLASS), key=lambda c: agg_ms[c])
         fl_top = tdgrad.model_flops(top, agg_q[top], agg_p[top])
@@ -205,20 +237,9 @@ def run_ours(args):
                         kernel="tdg_grad_kernel" + tdgrad.class_name(top), kernel_share_of_step=agg_ms[top] / ms,
                         peak_source="FP64 FMA-chain microbenchmark run live on this GPU (tdg_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                         whole_step_model_tflops=fl_all / (ms * 1e-3) * 1e-12, whole_step_frac=fl_all / (ms * 1e-3) * 1e-12 / peak_tf)
-        # end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region
-        hD, hP, hT = [x.cpu().pin_memory().numpy() for x in (D, P, T)]
-        hpairs, _, _ = wl.default_call(hD, hP, hT)
-        e2e_warm = 0 if ms / args.steps > 20000 else 1
-        for _ in range(e2e_warm):
-            step(hpairs, None, stats=False)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        g2, _ = step(hpairs, None, stats=False)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        assert np.max(np.abs(g2 - g_host)) < 1e-8, "host-buffer and device-buffer paths disagree"
+        dt = e2e_dt
         h2d = 3 * nbf * nbf * 8 + sysm.xyz.nbytes + sysm.exps.nbytes + sysm.coefs.nbytes + sysm.shells.nbytes
-        e2e = dict(value=(quartets / args.steps) / dt, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(natom * 3 * 8), seconds=dt)
+        e2e = dict(value=((total_quartets if shard else quartets) / args.steps) / dt, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(natom * 3 * 8), seconds=dt)
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             cpu = oracle_sample(cfg, sysm, (hD, hP, hT))
@@ -227,11 +248,11 @@ def run_ours(args):
                                                model_tflops=tdgrad.model_flops(c, agg_q[c], agg_p[c]) / (agg_ms[c] * 1e-3) * 1e-12)
                      for c in range(tdgrad.NCLASS) if agg_q[c]}
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms / args.steps,
-                    higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                    higher_is_better=True, scaling="strong" if shard else "weak", vs_baseline=None, dtype="f64", data="synthetic",
                     config=dict(workload=_workload_name(cfg), nbf=nbf, natom=natom, nshell=sysm.nshell, pairs=3, omega=wl.OMEGA,
                                 l2="inputs (3 x %.0f MB densities) larger than L2" % (nbf * nbf * 8 / 1e6),
-                                parallelism="replicas" if world > 1 else "1gpu"),
-                    wall_time_s=ms / args.steps * 1e-3, quartets_per_step=quartets // args.steps,
+                                parallelism=("shard%d+allreduce" % world) if shard else ("replicas" if world > 1 else "1gpu")),
+                    wall_time_s=ms / args.steps * 1e-3, quartets_per_step=total_quartets // args.steps,
                     grad_sum_abs_max=float(np.max(np.abs(g_host.sum(axis=0)))),
                     roofline=roofline, cpu_baseline=cpu, e2e=e2e, gpu_launches=launches, clocks=clocks, per_class=per_class)
         print(json.dumps(line))
@@ -248,6 +269,8 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "shard"],
+                    help="N > 1: independent replicas (weak scaling, default) or work items sharded over ranks + one NCCL all-reduce (strong)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -86,6 +86,15 @@ int tdg_nbf(const tdg_ctx* ctx, int* nbf);
  * Cached until tdg_set_system / tdg_plan is called again. */
 int tdg_plan(tdg_ctx* ctx, const tdg_options* opt);
 
+/* Multi-GPU sharding ("block-cyclic", 280-282, 304): this context computes only the
+ * (launch, bra tile) work items whose running index is congruent to `rank` modulo `nranks`; tiles within a bucket
+ * pair are ordered by Schwarz bound, so neighbouring items cost about the same and the deal balances.  The system,
+ * the pair plan and the densities stay replicated.  tdg_gradient / tdg_energy then return this rank's PARTIAL
+ * result and per-rank stats; the caller sums over ranks (one all-reduce of 3*natom doubles).  The union of the
+ * nranks shards is exactly the unsharded work list, each quartet on exactly one rank.  Default (0, 1).
+ * Invalidates the plan when the shard changes.  TDG_EINVAL unless 0 <= rank < nranks. */
+int tdg_set_shard(tdg_ctx* ctx, int rank, int nranks);
+
 /* Schwarz bounds of the current system: Q[nshell][nshell] to a HOST buffer (for tests/diagnostics). */
 int tdg_schwarz(tdg_ctx* ctx, double* Q_host);
 

@@ -59,6 +59,7 @@ struct tdg_ctx {
   std::vector<Bucket> buckets;
   std::vector<Work> work;
   int64_t pairs_total = 0, pairs_kept = 0;
+  int shard_rank = 0, shard_n = 1;   // tdg_set_shard: this context owns every shard_n-th (launch, bra tile) work item
   // per-call scratch
   double* d_grad = nullptr;
   double* d_dmax = nullptr;
@@ -127,6 +128,13 @@ extern "C" int tdg_destroy(tdg_ctx* ctx) {
   free_system(ctx);
   cudaFree(ctx->d_rys); cudaFree(ctx->d_counters);
   delete ctx;
+  return TDG_OK;
+}
+
+extern "C" int tdg_set_shard(tdg_ctx* ctx, int rank, int nranks) {
+  if (!ctx || nranks <= 0 || rank < 0 || rank >= nranks) return TDG_EINVAL;
+  if (rank != ctx->shard_rank || nranks != ctx->shard_n) { cudaSetDevice(ctx->device); free_plan(ctx); }
+  ctx->shard_rank = rank; ctx->shard_n = nranks;
   return TDG_OK;
 }
 
@@ -285,6 +293,7 @@ extern "C" int tdg_plan(tdg_ctx* ctx, const tdg_options* opt) {
     }
     // work lists: bucket b1 >= b2 (bucket order = (pair class, npp) ascending, so bra class >= ket class)
     const int nb = (int)ctx->buckets.size();
+    int64_t item = 0;   // running index of non-empty (launch, bra tile) work items, dealt round-robin over the ranks
     for (int b1 = 0; b1 < nb; ++b1)
       for (int b2 = 0; b2 <= b1; ++b2) {
         const Bucket& X = ctx->buckets[b1]; const Bucket& Y = ctx->buckets[b2];
@@ -297,6 +306,7 @@ extern "C" int tdg_plan(tdg_ctx* ctx, const tdg_options* opt) {
             klen = (int)(std::partition_point(Y.Q.begin(), Y.Q.end(), [&](double qk) { return qb * qk >= tau; }) - Y.Q.begin());
           }
           if (b1 == b2) klen = std::min(klen, std::min(X.n, (t + 1) * TDG_WARP));
+          if (klen > 0 && (item++ % ctx->shard_n) != ctx->shard_rank) klen = 0;   // another rank's tile: no blocks here
           cum[t + 1] = cum[t] + (klen + TDG_KB - 1) / TDG_KB;
         }
         if (cum[ntiles] == 0) continue;

@@ -1,0 +1,49 @@
+"""Load balance of the rank shards (tdg_set_shard) measured on ONE GPU: for each world size N the N
+shards run one after another, each to completion (no rank waits on another), and the device time of each is recorded.
+The predicted N-GPU step is the slowest shard; efficiency = unsharded time / (N x slowest shard).  The all-reduce of
+3*natom doubles (18 KB at cfg 3) is not in these numbers.
+
+    python -m paper_2407_16586_b200.shard_balance [config=3] [world sizes=2,4,8]
+"""
+import json
+import sys
+
+import numpy as np
+import torch
+
+from paper_2407_16586_b200 import tdgrad
+from paper_2407_16586_b200 import workload as wl
+
+
+def main():
+    cfg = int(sys.argv[1]) if len(sys.argv) > 1 else 3
+    worlds = [int(x) for x in (sys.argv[2] if len(sys.argv) > 2 else "2,4,8").split(",")]
+    ctx = tdgrad.Context(0)
+    s = wl.make_system(cfg)
+    ctx.set_system(s)
+    D, P, T = wl.make_densities_torch(s.nbf, 20240716 + cfg, "cuda")
+    pairs, wJ, wK = wl.default_call(D, P, T)
+
+    def run(rank, n):
+        ctx.set_shard(rank, n)
+        ctx.plan(s.tau, s.density_weighted)
+        g, st = ctx.gradient(pairs, wJ, wK, wl.C_J, wl.C_K, wl.C_LR, wl.OMEGA)
+        return g, st
+
+    run(0, 1)                      # warm-up
+    g1, st1 = run(0, 1)
+    out = dict(config=cfg, unsharded_ms=st1["ms_total"], quartets=st1["quartets_computed"], worlds=[])
+    for n in worlds:
+        ms, q, total = [], [], np.zeros_like(g1)
+        for r in range(n):
+            g, st = run(r, n)
+            ms.append(st["ms_total"]); q.append(st["quartets_computed"]); total += g
+        assert sum(q) == st1["quartets_computed"]
+        out["worlds"].append(dict(n=n, shard_ms=ms, shard_quartets=q, slowest_ms=max(ms), efficiency=st1["ms_total"] / (n * max(ms)),
+                                  max_abs_diff_vs_unsharded=float(np.max(np.abs(total - g1)))))
+    print(json.dumps(out))
+    ctx.close()
+
+
+if __name__ == "__main__":
+    main()

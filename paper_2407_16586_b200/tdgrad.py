@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libtdgrad.so")
 NCLASS = 55
 _lib = None
 
-SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_plan", "tdg_schwarz", "tdg_gradient",
+SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_shard", "tdg_plan", "tdg_schwarz", "tdg_gradient",
            "tdg_energy", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
 
 
@@ -99,6 +99,20 @@ def _ptr(x):
     return x.data_ptr()
 
 
+def shard_of_env():
+    """(rank, world size) of this process under torchrun (RANK / WORLD_SIZE), else (0, 1)."""
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def allreduce_partial(partial, group=None):
+    """Sum the per-rank partial gradients (torch tensor, in place) over the process group: the path's only exchange step."""
+    import torch.distributed as dist
+
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(partial, op=dist.ReduceOp.SUM, group=group)
+    return partial
+
+
 class Context:
     """One tdg_ctx on one CUDA device."""
 
@@ -141,6 +155,10 @@ class Context:
         self._check(lib().tdg_nbf(self._h, C.byref(n)), "tdg_nbf")
         return n.value
 
+    def set_shard(self, rank: int, nranks: int):
+        """This context computes the work items `rank` mod `nranks`; call before :meth:`plan`."""
+        self._check(lib().tdg_set_shard(self._h, C.c_int(rank), C.c_int(nranks)), "tdg_set_shard")
+
     def plan(self, tau=0.0, density_weighted=0, sample_mod=0, sample_seed=0):
         opt = Options(tau, density_weighted, sample_mod, sample_seed)
         self._check(lib().tdg_plan(self._h, C.byref(opt)), "tdg_plan")
@@ -180,6 +198,13 @@ class Context:
                                 C.byref(st) if st is not None else None)
         self._check(rc, "tdg_gradient")
         return g, (st.asdict() if st is not None else None)
+
+    def gradient_allreduce(self, pairs, wJ, wK, cJ, cK, cLR, omega, out, group=None, stream=None):
+        """Sharded gradient: this rank's partial gradient from the CUDA kernels into the
+        CUDA tensor ``out`` [natom, 3], then ONE all-reduce (sum) of its 3*natom doubles over ``group`` (NCCL when the
+        tensors are on the GPU).  Requires :meth:`set_shard` (rank, world size) before :meth:`plan`.  No arithmetic here."""
+        g, _ = self.gradient(pairs, wJ, wK, cJ, cK, cLR, omega, stream=stream, out=out, want_stats=False)
+        return allreduce_partial(g, group)
 
     def energy(self, pairs, wJ, wK, cJ, cK, cLR, omega, stream=None) -> float:
         """Contracted energy E (host float) for the same arguments as :meth:`gradient` (untuned; for FD checks)."""

@@ -228,3 +228,44 @@ def test_cfg4_subsample_largest_configuration(ctx, orc):
     _compare(g, ref)
     assert st["pairs_kept"] == rst["pairs_kept"]
     assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 3
+
+
+@pytest.mark.parametrize("nranks", [2, 3])
+def test_sharded_work_items_partition_the_gradient(ctx, orc, nranks):
+    """SURVEY.md 8(e) / PAPER.md:309: the rank shards (tdg_set_shard) partition the quartets exactly (integer counts add up
+    to the unsharded ones, class by class) and their partial gradients sum to the oracle's gradient.  The shards run one
+    after another on this GPU, each to completion; no rank waits on another."""
+    s = wl.make_system(1)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    try:
+        g_full, st_full, ref, _ = _run_both(ctx, orc, s, pairs, wJ, wK)
+        total = np.zeros_like(g_full)
+        counts = {k: 0 for k in ("quartets_visited", "quartets_computed", "prim_quartets")}
+        by_class = np.zeros(len(st_full["quartets_by_class"]), dtype=np.int64)
+        for r in range(nranks):
+            ctx.set_shard(r, nranks)
+            ctx.plan(s.tau, s.density_weighted)
+            g, st = ctx.gradient(pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"])
+            assert 0 < st["quartets_computed"] < st_full["quartets_computed"]
+            assert st["quartets_computed"] < 1.5 * st_full["quartets_computed"] / nranks   # the deal balances
+            total += g
+            for k in counts:
+                counts[k] += st[k]
+            by_class += np.asarray(st["quartets_by_class"], dtype=np.int64)
+        for k in counts:
+            assert counts[k] == st_full[k], (k, counts[k], st_full[k])
+        assert np.array_equal(by_class, np.asarray(st_full["quartets_by_class"], dtype=np.int64))
+        _compare(total, ref)
+        _compare(total, g_full)
+    finally:
+        ctx.set_shard(0, 1)
+
+
+def test_set_shard_rejects_bad_arguments(ctx):
+    from paper_2407_16586_b200 import tdgrad
+
+    for rank, n in ((-1, 2), (2, 2), (0, 0)):
+        with pytest.raises(tdgrad.TdgError):
+            ctx.set_shard(rank, n)
+    ctx.set_shard(0, 1)
