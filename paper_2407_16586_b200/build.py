@@ -19,6 +19,7 @@ QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASS
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-DTDG_LMAX_BUILD=%d" % LMAX]
+CLASS_FLAGS = {}   # per-class overrides of the role split (tdg_grad.cuh: TDG_ROLE_COMPS, TDG_MAX_ROLES), measured on cfg 3
 DEPS = {   # headers each source includes
     "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "rys_meta.inc"],
     "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
@@ -44,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     jobs = [("tdg_api.cu", os.path.join(OBJ, "tdg_api.o"), []), ("tdg_aux.cu", os.path.join(OBJ, "tdg_aux.o"), [])]
     for la, lb, lc, ld in QUARTET_CLASSES:
         jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d%d%d.o" % (la, lb, lc, ld)),
-                     ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb, "-DTDG_LC=%d" % lc, "-DTDG_LD=%d" % ld]))
+                     ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb, "-DTDG_LC=%d" % lc, "-DTDG_LD=%d" % ld] + CLASS_FLAGS.get((la, lb, lc, ld), [])))
     # longest compiles first (fully unrolled d-shell classes)
     jobs.sort(key=lambda j: 0 if "class" not in j[1] else -sum(int(c) for c in os.path.basename(j[1])[10:14]))
     todo = []
