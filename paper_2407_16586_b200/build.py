@@ -19,7 +19,9 @@ QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASS
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-DTDG_LMAX_BUILD=%d" % LMAX]
-CLASS_FLAGS = {}   # per-class overrides of the role split (tdg_grad.cuh: TDG_ROLE_COMPS, TDG_MAX_ROLES), measured on cfg 3
+# per-class overrides of the role split (tdg_grad.cuh: TDG_ROLE_COMPS, TDG_MAX_ROLES), measured on cfg 3:
+# (dd|dp) with 54 function quartets per role = 12 roles, fully unrolled: 1067 ms -> 110 ms (this one object takes ~14 min to compile)
+CLASS_FLAGS = {(2, 2, 2, 1): ["-DTDG_ROLE_COMPS=54"]}
 DEPS = {   # headers each source includes
     "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "rys_meta.inc"],
     "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
