@@ -27,7 +27,10 @@
  * integrals vs high-precision differentiation of the (ss|ss) closed form; unit self-overlap;
  * omega->infinity and omega->0 limits; derivative integrals vs finite differences; gradient vs
  * central finite differences of orc_energy; sum_A g_A = 0; N^4 loop vs unique-quartet loop;
- * K(T,T) vs explicit MO sum; energy vs numpy einsum over orc_eri_tensor.
+ * K(T,T) vs explicit MO sum; energy vs numpy einsum over orc_eri_tensor; the density-weighted
+ * screening rule (density_maxima, quartet_weight) vs the Cauchy-Schwarz inequality on every
+ * density-weighted integral, the closed form for s shells, permutation/transpose invariance and
+ * the c * n_dropped * tau error bound (tests/test_oracle_screening.py).
  * Paper-printed values: none exist for this path ("parity unpinned" w.r.t. printed numbers).
  */
 #include <math.h>
@@ -521,6 +524,37 @@ static void density_maxima(const sys_t *s, int nmat, const double *const *M, dou
         }
 }
 
+/* S9: W_ijkl = max(C_J d_ij d_kl, C_K max(d_ik d_jl, d_il d_jk)) from the shell-block maxima d[ns][ns]. */
+static double quartet_weight(const double *dm, int ns, int i, int j, int k, int l, double CJ, double CK) {
+    double dij = dm[(size_t)i * ns + j], dkl = dm[(size_t)k * ns + l];
+    double dik = dm[(size_t)i * ns + k], djl = dm[(size_t)j * ns + l];
+    double dil = dm[(size_t)i * ns + l], djk = dm[(size_t)j * ns + k];
+    double x1 = dik * djl, x2 = dil * djk;
+    double W = CJ * dij * dkl, WK = CK * (x1 > x2 ? x1 : x2);
+    if (WK > W) W = WK;
+    return W;
+}
+
+/* Test access to the two S9 quantities above (tests/test_oracle_screening.py pins them): d[ns][ns] of the 2*npair
+ * matrices A_k, B_k, and W[ns][ns][ns][ns] with C_J = sum|wJ_k cJ|, C_K = (|cK|+|cLR|) sum|wK_k| as in contract_driver. */
+int orc_density_weights(SYS_ARGS, int npair, const double *const *A, const double *const *B, const double *wJ,
+                        const double *wK, double cJ, double cK, double cLR, double *d, double *W) {
+    sys_t s; int rc = sys_init(&s, SYS_PASS); if (rc) return rc;
+    int ns = nshell;
+    double CJ = 0.0, CK = 0.0;
+    for (int k = 0; k < npair; ++k) { CJ += fabs(wJ[k] * cJ); CK += fabs(wK[k]); }
+    CK *= fabs(cK) + fabs(cLR);
+    const double **M = (const double **)malloc(sizeof(double *) * 2 * (size_t)npair);
+    for (int k = 0; k < npair; ++k) { M[2 * k] = A[k]; M[2 * k + 1] = B[k]; }
+    density_maxima(&s, 2 * npair, M, d);
+    free(M);
+    if (W)
+        for (int i = 0; i < ns; ++i) for (int j = 0; j < ns; ++j) for (int k = 0; k < ns; ++k) for (int l = 0; l < ns; ++l)
+            W[(((size_t)i * ns + j) * ns + k) * ns + l] = quartet_weight(d, ns, i, j, k, l, CJ, CK);
+    sys_free(&s);
+    return 0;
+}
+
 typedef struct { int i, j; double Q; } pair_t;
 static int pair_cmp(const void *a, const void *b) {
     const pair_t *x = (const pair_t *)a, *y = (const pair_t *)b;
@@ -600,15 +634,7 @@ static int contract_driver(int mode, SYS_ARGS, const orc_options *opt, int npair
                     double qq = Qij * pairs[pb].Q;
                     if (qq < tau) break;
                     ++visited;
-                    if (dw) {
-                        double dij = dm[(size_t)i * ns + j], dkl = dm[(size_t)k * ns + l];
-                        double dik = dm[(size_t)i * ns + k], djl = dm[(size_t)j * ns + l];
-                        double dil = dm[(size_t)i * ns + l], djk = dm[(size_t)j * ns + k];
-                        double x1 = dik * djl, x2 = dil * djk;
-                        double W = CJ * dij * dkl, WK = CK * (x1 > x2 ? x1 : x2);
-                        if (WK > W) W = WK;
-                        if (qq * W < tau) continue;
-                    }
+                    if (dw && qq * quartet_weight(dm, ns, i, j, k, l, CJ, CK) < tau) continue;
                 } else ++visited;
                 if (!sample_keep(i, j, k, l, smod, sseed)) continue;
                 ++computed;

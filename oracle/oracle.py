@@ -158,6 +158,22 @@ def gradient_n4(sysm, pairs, wJ, wK, cJ, cK, cLR, omega):
     return out.reshape(-1, 3)
 
 
+def density_weights(sysm, pairs, wJ, wK, cJ, cK, cLR, want_W=True):
+    """S9 quantities as the oracle's screening uses them: d[ns, ns] and (optionally) W[ns, ns, ns, ns]."""
+    args, keep = _sys_args(sysm)
+    PA, PB, keep2 = _mats(pairs)
+    wJ = np.ascontiguousarray(wJ, dtype=np.float64)
+    wK = np.ascontiguousarray(wK, dtype=np.float64)
+    ns = sysm.nshell
+    d = np.zeros((ns, ns))
+    W = np.zeros((ns, ns, ns, ns)) if want_W else None
+    rc = lib().orc_density_weights(*args, C.c_int(len(pairs)), PA, PB, wJ.ctypes.data_as(C.c_void_p), wK.ctypes.data_as(C.c_void_p),
+                                   C.c_double(cJ), C.c_double(cK), C.c_double(cLR), d.ctypes.data_as(C.c_void_p),
+                                   W.ctypes.data_as(C.c_void_p) if want_W else None)
+    assert rc == 0, rc
+    return d, W
+
+
 def sample_keep(i, j, k, l, mod, seed) -> bool:
     return bool(lib().orc_sample_keep(C.c_int(i), C.c_int(j), C.c_int(k), C.c_int(l), C.c_uint32(mod), C.c_uint32(seed)))
 
