@@ -68,6 +68,7 @@ typedef struct {
   float ms_prepare;                    /* density preparation (a3)                                        */
   float ms_total;                      /* whole tdg_gradient device time                                  */
   int32_t launches;                    /* kernels launched by this call                                   */
+  int32_t groups;                      /* passes over the class kernels (1 unless the pairs need > 4 canonical matrices) */
 } tdg_stats;
 
 /* Create a context on CUDA device `cuda_device`.  TDG_ECUDA if there is none. */
@@ -95,6 +96,11 @@ int tdg_plan(tdg_ctx* ctx, const tdg_options* opt);
  * Invalidates the plan when the shard changes.  TDG_EINVAL unless 0 <= rank < nranks. */
 int tdg_set_shard(tdg_ctx* ctx, int rank, int nranks);
 
+/* Class launches of one tdg_gradient call are independent; with nstreams > 1 they are dealt over the caller's stream and
+ * nstreams-1 internal streams that fork from / join it by events, so the call stays stream-ordered for the caller.
+ * Per-class times in tdg_stats then overlap (their sum exceeds ms_total).  1 <= nstreams <= 8; default 1. */
+int tdg_set_streams(tdg_ctx* ctx, int nstreams);
+
 /* Schwarz bounds of the current system: Q[nshell][nshell] to a HOST buffer (for tests/diagnostics). */
 int tdg_schwarz(tdg_ctx* ctx, double* Q_host);
 
@@ -104,7 +110,9 @@ int tdg_schwarz(tdg_ctx* ctx, double* Q_host);
  * stream: cudaStream_t (as void*) or NULL for the default stream.
  * grad: [natom][3], device pointer if `grad_on_device` != 0 (completion is then stream-ordered) else host
  * (the call synchronises).  Overwritten, not accumulated.  stats may be NULL (non-NULL adds per-class
- * event timing and synchronises). */
+ * event timing and synchronises; the quartet counters are only read back then).
+ * The call blocks the host ONCE mid-way when exchange is on (cK or cLR != 0 and some wK != 0): it reads back which
+ * inputs are nonsymmetric, because that decides how many canonical matrices are packed (reading R1). */
 int tdg_gradient(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
                  const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
                  void* stream, double* grad, int grad_on_device, tdg_stats* stats);

@@ -19,11 +19,10 @@ QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASS
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
          "-DTDG_LMAX_BUILD=%d" % LMAX]
-# per-class overrides of the role split (tdg_grad.cuh: TDG_ROLE_COMPS, TDG_MAX_ROLES), measured on cfg 3:
-# (dd|dp) with 54 function quartets per role = 12 roles, fully unrolled: 1067 ms -> 110 ms (this one object takes ~14 min to compile)
-CLASS_FLAGS = {(2, 2, 2, 1): ["-DTDG_ROLE_COMPS=54"]}
+# per-class compile flags (launch bounds measured on cfg 3, see profiles/): class -> extra nvcc flags
+CLASS_FLAGS: dict = {}
 DEPS = {   # headers each source includes
-    "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "rys_meta.inc"],
+    "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "rys_meta.inc"],
     "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
     "tdg_api.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "../../include/tdgrad.h"],
 }
@@ -35,11 +34,20 @@ def _newest_header(src: str) -> float:
 
 def _compile(job):
     src, obj, extra = job
-    cmd = [NVCC] + FLAGS + os.environ.get("TDG_EXTRA_FLAGS", "").split() + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
+    cmd = [NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    with open(obj + ".cmd", "w") as f:   # an object is stale when its flags change, not only when its sources do
+        f.write(" ".join(FLAGS + extra))
     return obj
+
+
+def _same_flags(obj, extra) -> bool:
+    try:
+        return open(obj + ".cmd").read() == " ".join(FLAGS + extra)
+    except OSError:
+        return False
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -53,12 +61,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     todo = []
     for src, obj, extra in jobs:
         st = max(os.path.getmtime(os.path.join(CSRC, src)), _newest_header(src))
-        if force or not os.path.exists(obj) or os.path.getmtime(obj) < st:
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < st or not _same_flags(obj, extra):
             todo.append((src, obj, extra))
-    only = os.environ.get("TDG_ONLY")   # developer aid: recompile only these classes (e.g. "1000,1110"), reuse the other objects
-    if only:
-        keep = tuple("tdg_class_%s.o" % c for c in only.split(","))
-        todo = [j for j in jobs if j[1].endswith(keep) or not os.path.exists(j[1])]
     if todo:
         if verbose:
             print("compiling %d objects" % len(todo), file=sys.stderr)

@@ -13,6 +13,7 @@
 #include "tdg_internal.h"
 
 #define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
+#define TDG_MAX_STREAMS 8
 
 #define TDG_CLASS(la, lb, lc, ld) tdg_launch_fn tdg_class_launcher_##la##lb##lc##ld();
 #include "tdg_classes.inc"
@@ -33,7 +34,6 @@ struct Bucket {       // shell pairs of one (la, lb, primitive-pair count), sort
   PairHdr* d_hdr = nullptr;
   double* d_prim = nullptr;
   std::vector<double> Q;   // host copy of the sorted bounds
-  std::vector<int> last_same;  // unused
 };
 struct Work {         // one kernel launch: bra bucket x ket bucket
   int b1, b2, cls, nblocks, ntiles;
@@ -60,6 +60,9 @@ struct tdg_ctx {
   std::vector<Work> work;
   int64_t pairs_total = 0, pairs_kept = 0;
   int shard_rank = 0, shard_n = 1;   // tdg_set_shard: this context owns every shard_n-th (launch, bra tile) work item
+  int nstreams = 1;                  // tdg_set_streams: class launches are dealt over the caller's stream + nstreams-1 side streams
+  cudaStream_t side[TDG_MAX_STREAMS - 1] = {};
+  cudaEvent_t ev_fork = nullptr, ev_join[TDG_MAX_STREAMS - 1] = {};
   // per-call scratch
   double* d_grad = nullptr;
   double* d_dmax = nullptr;
@@ -92,7 +95,7 @@ static void free_system(tdg_ctx* c) {
   c->d_xyz = c->d_exps = c->d_cn = c->d_Q = c->d_grad = c->d_dmax = nullptr; c->d_shells = nullptr;
   for (auto& s : c->scratch) cudaFree(s.second);
   c->scratch.clear(); c->scratch_used.clear();
-  c->have_Q = false; c->nshell = 0;
+  c->have_Q = false; c->nshell = 0; c->natom = 0; c->nbf = 0; c->nprim = 0;
 }
 
 extern "C" const char* tdg_strerror(int code) {
@@ -127,6 +130,11 @@ extern "C" int tdg_destroy(tdg_ctx* ctx) {
   cudaSetDevice(ctx->device);
   free_system(ctx);
   cudaFree(ctx->d_rys); cudaFree(ctx->d_counters);
+  for (int i = 0; i < TDG_MAX_STREAMS - 1; ++i) {
+    if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
+    if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+  }
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   delete ctx;
   return TDG_OK;
 }
@@ -135,6 +143,18 @@ extern "C" int tdg_set_shard(tdg_ctx* ctx, int rank, int nranks) {
   if (!ctx || nranks <= 0 || rank < 0 || rank >= nranks) return TDG_EINVAL;
   if (rank != ctx->shard_rank || nranks != ctx->shard_n) { cudaSetDevice(ctx->device); free_plan(ctx); }
   ctx->shard_rank = rank; ctx->shard_n = nranks;
+  return TDG_OK;
+}
+
+extern "C" int tdg_set_streams(tdg_ctx* ctx, int nstreams) {
+  if (!ctx || nstreams < 1 || nstreams > TDG_MAX_STREAMS) return TDG_EINVAL;
+  cudaSetDevice(ctx->device);
+  if (!ctx->ev_fork) CK(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+  for (int i = 0; i < nstreams - 1; ++i) {
+    if (!ctx->side[i]) CK(cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
+    if (!ctx->ev_join[i]) CK(cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming));
+  }
+  ctx->nstreams = nstreams;
   return TDG_OK;
 }
 
@@ -157,13 +177,9 @@ extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int ns
     if (sh.l > TDG_MAX_L || sh.l > TDG_LMAX_BUILD) return TDG_EUNSUPPORTED;
     for (int k = 0; k < sh.nprim; ++k) if (!(exps[sh.prim_off + k] > 0.0)) return TDG_EINVAL;
   }
-  cudaSetDevice(ctx->device);
-  free_system(ctx);
-  ctx->natom = natom; ctx->nshell = nshell; ctx->nprim = nprim_total;
-  ctx->xyz.assign(xyz, xyz + 3 * (size_t)natom);
-  ctx->exps.assign(exps, exps + nprim_total);
-  ctx->cn.assign(nprim_total, 0.0);
-  ctx->shells.resize(nshell);
+  // a0: all host arithmetic and validation first; the context is only touched once nothing can fail on the host side
+  std::vector<double> cn(nprim_total, 0.0);
+  std::vector<DevShell> dsh(nshell);
   int off = 0;
   const double PI = 3.14159265358979323846;
   for (int s = 0; s < nshell; ++s) {
@@ -177,12 +193,17 @@ extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int ns
     if (!(S > 0.0)) return TDG_EINVAL;
     for (int k = 0; k < sh.nprim; ++k) {
       const double z = exps[sh.prim_off + k];
-      ctx->cn[sh.prim_off + k] = coefs[sh.prim_off + k] * std::pow(2.0 * z / PI, 0.75) * std::pow(4.0 * z, 0.5 * sh.l) / std::sqrt(S);
+      cn[sh.prim_off + k] = coefs[sh.prim_off + k] * std::pow(2.0 * z / PI, 0.75) * std::pow(4.0 * z, 0.5 * sh.l) / std::sqrt(S);
     }
-    ctx->shells[s] = DevShell{sh.atom, sh.l, sh.nprim, sh.prim_off, off, 0};
+    dsh[s] = DevShell{sh.atom, sh.l, sh.nprim, sh.prim_off, off, 0};
     off += ncart(sh.l);
   }
-  ctx->nbf = off;
+  cudaSetDevice(ctx->device);
+  free_system(ctx);   // leaves the context empty (nshell = 0): a failed upload below cannot leave a half-initialised system behind
+  ctx->xyz.assign(xyz, xyz + 3 * (size_t)natom);
+  ctx->exps.assign(exps, exps + nprim_total);
+  ctx->cn = std::move(cn);
+  ctx->shells = std::move(dsh);
   {
     std::vector<int> bf2sh(off);
     for (int sidx = 0; sidx < nshell; ++sidx)
@@ -200,6 +221,8 @@ extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int ns
   CK(cudaMemcpy(ctx->d_exps, ctx->exps.data(), sizeof(double) * nprim_total, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(ctx->d_cn, ctx->cn.data(), sizeof(double) * nprim_total, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(ctx->d_shells, ctx->shells.data(), sizeof(DevShell) * nshell, cudaMemcpyHostToDevice));
+  // only now does the context count as holding a system (tdg_plan / tdg_schwarz check nshell > 0)
+  ctx->natom = natom; ctx->nshell = nshell; ctx->nprim = nprim_total; ctx->nbf = off;
   return TDG_OK;
 }
 
@@ -281,8 +304,8 @@ extern "C" int tdg_plan(tdg_ctx* ctx, const tdg_options* opt) {
             double* r = pp + (size_t)(ka * sb.nprim + kb) * TDG_PRIM_STRIDE;
             r[0] = p;
             for (int d = 0; d < 3; ++d) r[1 + d] = (a * A[d] + b * Bc[d]) / p;
-            r[4] = ctx->cn[sa.prim_off + ka] * ctx->cn[sb.prim_off + kb] * std::exp(-a * b / p * R2);
-            r[5] = a; r[6] = b; r[7] = 0.0;
+            r[4] = ctx->cn[sa.prim_off + ka] * ctx->cn[sb.prim_off + kb] * std::exp(-a * b / p * R2) / p;
+            r[5] = a; r[6] = b; r[7] = 1.0 / p;
           }
       }
       CK(cudaMalloc(&B.d_hdr, sizeof(PairHdr) * hdr.size()));
@@ -341,6 +364,15 @@ static void* scratch_get(tdg_ctx* ctx, size_t bytes) {
 
 namespace {
 struct Group { std::vector<int> pairs; std::vector<int> canon; };   // canonical matrix id = 2*unique + (0: sym part, 1: antisym part)
+struct EventPool {   // timing events of one call; destroyed on every exit path
+  std::vector<cudaEvent_t> v;
+  cudaEvent_t get() { cudaEvent_t e = nullptr; if (cudaEventCreate(&e) == cudaSuccess) v.push_back(e); return e; }
+  ~EventPool() { for (cudaEvent_t e : v) cudaEventDestroy(e); }
+};
+struct DevTemp {     // cudaMalloc'ed temporary freed on every exit path
+  void* p = nullptr;
+  ~DevTemp() { cudaFree(p); }
+};
 }
 
 static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int on_dev,
@@ -349,8 +381,9 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
   const int n = ctx->nbf;
   const size_t mbytes = sizeof(double) * (size_t)n * n;
   std::fill(ctx->scratch_used.begin(), ctx->scratch_used.end(), false);
+  EventPool pool;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
-  if (stats) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventCreate(&ev2); cudaEventRecord(ev0, st); }
+  if (stats) { ev0 = pool.get(); ev1 = pool.get(); ev2 = pool.get(); if (!ev0 || !ev1 || !ev2) return TDG_ECUDA; cudaEventRecord(ev0, st); }
   // unique input matrices -> device pointers
   std::vector<const double*> uniq, udev;
   auto uid = [&](const double* M) { for (size_t i = 0; i < uniq.size(); ++i) if (uniq[i] == M) return (int)i; return -1; };
@@ -402,16 +435,15 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
   P.CJ = CJ; P.CK = CKs;
   P.tau = ctx->opt.tau; P.density_weighted = (ctx->opt.tau > 0.0) ? ctx->opt.density_weighted : 0;
   P.nshell = ctx->nshell; P.sample_mod = ctx->opt.sample_mod; P.sample_seed = ctx->opt.sample_seed;
-  P.nbf = n; P.cK = cK; P.cLR = cLR; P.omega2 = omega * omega; P.use_lr = (cLR != 0.0) ? 1 : 0;
+  P.nbf = n; P.cK = cK; P.cLR = cLR; P.omega = omega; P.omega2 = omega * omega; P.use_lr = (cLR != 0.0) ? 1 : 0;
   P.grad = ctx->d_grad; P.rys_tab = ctx->d_rys;
   int aux_launches = (int)uniq.size();
   if (P.density_weighted) {   // d_ij over ALL input matrices (reading S9)
     if (!ctx->d_dmax) CK(cudaMalloc(&ctx->d_dmax, sizeof(double) * (size_t)ctx->nshell * ctx->nshell));
-    const double** d_list = (const double**)scratch_get(ctx, 512);
-    if (!d_list) return TDG_ENOMEM;
-    CK(cudaMemcpyAsync(d_list, udev.data(), sizeof(double*) * udev.size(), cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));
-    CK(tdg_launch_dmax(d_list, (int)udev.size(), n, ctx->d_shells, ctx->nshell, ctx->d_dmax, st));
+    MatList ml{};
+    ml.n = (int)udev.size();
+    for (int i = 0; i < ml.n; ++i) ml.m[i] = udev[i];
+    CK(tdg_launch_dmax(ml, n, ctx->d_shells, ctx->nshell, ctx->d_dmax, st));
     P.dmax = ctx->d_dmax;
     aux_launches += 2;
   }
@@ -429,8 +461,9 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
   CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * (nw * 3 + 3), st));
   if (stats) cudaEventRecord(ev1, st);
   int launches = 0;
-  std::vector<cudaEvent_t> evs;
+  std::vector<cudaEvent_t> evs;   // (start, stop) per launch, on the launch's own stream
   std::vector<int> ev_cls;
+  const int nstr = d_E ? 1 : ctx->nstreams;
   for (size_t gi = 0; gi < groups.size(); ++gi) {
     const Group& G = groups[gi];
     PackSrc ps{};
@@ -450,6 +483,12 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
         P.MK[4 * na + nb] += wk; P.MK[4 * nb + na] += wk;
       }
     }
+    // class launches are independent (they only add into grad and their own counters): deal them over the streams so
+    // that the under-filled tail of one launch overlaps the next; the side streams fork from and join the caller's
+    if (nstr > 1) {
+      CK(cudaEventRecord(ctx->ev_fork, st));
+      for (int i = 0; i < nstr - 1; ++i) CK(cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
+    }
     for (size_t w = 0; w < nw; ++w) {
       const Work& W = ctx->work[w];
       const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
@@ -459,11 +498,17 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
       P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
       P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
       P.counters = ctx->d_counters + 3 * (gi == 0 ? w : nw);   // quartet counts come from the first group only
-      if (stats) { cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, st); evs.push_back(e); ev_cls.push_back(W.cls); }
-      if (d_E) CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, st));
-      else fn(P, W.nblocks, st);
+      const int si = (int)(w % (size_t)nstr);
+      cudaStream_t ls = si == 0 ? st : ctx->side[si - 1];
+      cudaEvent_t e0 = nullptr, e1 = nullptr;
+      if (stats) { e0 = pool.get(); e1 = pool.get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, ls); }
+      if (d_E) CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, ls));
+      else fn(P, W.nblocks, ls);
+      if (stats) { cudaEventRecord(e1, ls); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(W.cls); }
       ++launches;
     }
+    if (nstr > 1)
+      for (int i = 0; i < nstr - 1; ++i) { CK(cudaEventRecord(ctx->ev_join[i], ctx->side[i])); CK(cudaStreamWaitEvent(st, ctx->ev_join[i], 0)); }
   }
   CK(cudaGetLastError());
   if (d_E) {
@@ -483,16 +528,15 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
       stats->quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 1];
       stats->prim_quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 2];
     }
-    for (size_t e = 0; e < evs.size(); ++e) {
+    for (size_t e = 0; e < ev_cls.size(); ++e) {
       float ms = 0.f;
-      cudaEventElapsedTime(&ms, evs[e], e + 1 < evs.size() ? evs[e + 1] : ev2);
+      cudaEventElapsedTime(&ms, evs[2 * e], evs[2 * e + 1]);
       stats->ms_by_class[ev_cls[e]] += ms;
     }
     cudaEventElapsedTime(&stats->ms_prepare, ev0, ev1);
     cudaEventElapsedTime(&stats->ms_total, ev0, ev2);
     stats->launches = launches + aux_launches;
-    for (auto e : evs) cudaEventDestroy(e);
-    cudaEventDestroy(ev0); cudaEventDestroy(ev1); cudaEventDestroy(ev2);
+    stats->groups = (int32_t)groups.size();
   }
   return TDG_OK;
 }
@@ -530,14 +574,13 @@ extern "C" int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const
 extern "C" int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out) {
   if (!ctx || !T || !rho || !out || n < 1 || n > 7 || count <= 0) return TDG_EINVAL;
   cudaSetDevice(ctx->device);
-  double *dT = nullptr, *dr = nullptr, *dout = nullptr;
-  CK(cudaMalloc(&dT, sizeof(double) * count)); CK(cudaMalloc(&dr, sizeof(double) * count));
-  CK(cudaMalloc(&dout, sizeof(double) * (size_t)count * 2 * n));
-  CK(cudaMemcpy(dT, T, sizeof(double) * count, cudaMemcpyHostToDevice));
-  CK(cudaMemcpy(dr, rho, sizeof(double) * count, cudaMemcpyHostToDevice));
-  CK(tdg_launch_rys(n, count, dT, dr, omega, ctx->d_rys, dout, 0));
-  CK(cudaMemcpy(out, dout, sizeof(double) * (size_t)count * 2 * n, cudaMemcpyDeviceToHost));
-  cudaFree(dT); cudaFree(dr); cudaFree(dout);
+  DevTemp dT, dr, dout;
+  CK(cudaMalloc(&dT.p, sizeof(double) * count)); CK(cudaMalloc(&dr.p, sizeof(double) * count));
+  CK(cudaMalloc(&dout.p, sizeof(double) * (size_t)count * 2 * n));
+  CK(cudaMemcpy(dT.p, T, sizeof(double) * count, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(dr.p, rho, sizeof(double) * count, cudaMemcpyHostToDevice));
+  CK(tdg_launch_rys(n, count, (const double*)dT.p, (const double*)dr.p, omega, ctx->d_rys, (double*)dout.p, 0));
+  CK(cudaMemcpy(out, dout.p, sizeof(double) * (size_t)count * 2 * n, cudaMemcpyDeviceToHost));
   return TDG_OK;
 }
 

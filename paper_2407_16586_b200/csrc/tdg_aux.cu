@@ -174,7 +174,7 @@ __device__ static double quartet_energy(const KParams& P, int la, int lb, int lc
       const double PQx = Px - Qx, PQy = Py - Qy, PQz = Pz - Qz;
       const double rpq = 1.0 / (p + q), rho = p * q * rpq;
       const double T = rho * (PQx * PQx + PQy * PQy + PQz * PQz);
-      const double pref = 34.986836655249725693 * Kab * Kcd * rpq * sqrt(rpq) / rho;
+      const double pref = 34.986836655249725693 * Kab * Kcd * sqrt(rpq);   // records hold K_ab/p, K_cd/q
       for (int op = 0; op <= P.use_lr; ++op) {
         double s2 = 1.0, ss = 1.0;
         if (op == 1) { s2 = P.omega2 / (P.omega2 + rho); ss = sqrt(s2); }
@@ -298,29 +298,6 @@ cudaError_t tdg_launch_asym(const double* M, int n, double* out, cudaStream_t s)
   return cudaGetLastError();
 }
 
-__global__ void symsplit_kernel(const double* __restrict__ M, int n, double* __restrict__ S, double* __restrict__ N) {
-  __shared__ double tile[32][33];
-  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
-  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-    const int row = bx + r, col = by + threadIdx.x;
-    tile[r][threadIdx.x] = (row < n && col < n) ? M[(size_t)row * n + col] : 0.0;   // M[bx+r][by+c]
-  }
-  __syncthreads();
-  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-    const int row = by + r, col = bx + threadIdx.x;
-    if (row < n && col < n) {
-      const double a = M[(size_t)row * n + col], b = tile[threadIdx.x][r];       // M[row][col], M[col][row]
-      S[(size_t)row * n + col] = 0.5 * (a + b);
-      N[(size_t)row * n + col] = 0.5 * (a - b);
-    }
-  }
-}
-cudaError_t tdg_launch_symsplit(const double* M, int n, double* S, double* N, cudaStream_t s) {
-  dim3 block(32, 8), grid((n + 31) / 32, (n + 31) / 32);
-  symsplit_kernel<<<grid, block, 0, s>>>(M, n, S, N);
-  return cudaGetLastError();
-}
-
 __global__ void pack_kernel(const PackSrc ps, int n, const int* __restrict__ bf2sh, const DevShell* __restrict__ sh,
                             double* __restrict__ pk) {
   const int col = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
@@ -346,15 +323,14 @@ cudaError_t tdg_launch_pack(const PackSrc& ps, int n, const int* bf2sh, const De
   return cudaGetLastError();
 }
 
-__global__ void dmax_block_kernel(const double* const* __restrict__ mats, int nmat, int n, const DevShell* __restrict__ sh,
-                                  int ns, double* __restrict__ m) {
+__global__ void dmax_block_kernel(const MatList mats, int n, const DevShell* __restrict__ sh, int ns, double* __restrict__ m) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
   if (j >= ns) return;
   const DevShell si = sh[i], sj = sh[j];
   const int ni = ncart(si.l), nj = ncart(sj.l);
   double mx = 0.0;
-  for (int q = 0; q < nmat; ++q) {
-    const double* M = mats[q];
+  for (int q = 0; q < mats.n; ++q) {
+    const double* M = mats.m[q];
     for (int a = 0; a < ni; ++a)
       for (int b = 0; b < nj; ++b) {
         const double v = fabs(M[(size_t)(si.bf_off + a) * n + sj.bf_off + b]);
@@ -371,9 +347,9 @@ __global__ void dmax_sym_kernel(int ns, double* __restrict__ m) {
   m[(size_t)i * ns + j] = v;
   m[(size_t)j * ns + i] = v;
 }
-cudaError_t tdg_launch_dmax(const double* const* mats_dev, int nmat, int n, const DevShell* sh, int ns, double* m, cudaStream_t s) {
+cudaError_t tdg_launch_dmax(const MatList& mats, int n, const DevShell* sh, int ns, double* m, cudaStream_t s) {
   dim3 block(128), grid((ns + 127) / 128, ns);
-  dmax_block_kernel<<<grid, block, 0, s>>>(mats_dev, nmat, n, sh, ns, m);
+  dmax_block_kernel<<<grid, block, 0, s>>>(mats, n, sh, ns, m);
   dmax_sym_kernel<<<grid, block, 0, s>>>(ns, m);
   return cudaGetLastError();
 }

@@ -19,7 +19,7 @@ struct __align__(16) PairHdr {
   int32_t atomA, atomB;
   int32_t offA, offB;    // first basis function of each shell
 };
-// Primitive-pair record: 8 doubles: p, Px, Py, Pz, Kab, a, b, (unused)
+// Primitive-pair record: 8 doubles: p, Px, Py, Pz, K_ab/p, a, b, 1/p   (K_ab = c_a c_b exp(-ab/p |AB|^2), coefficients of step a0)
 #define TDG_PRIM_STRIDE 8
 
 
@@ -36,7 +36,7 @@ struct KParams {
   // (MJ, MK symmetric 4x4: sum over density pairs of w (e_x e_y^T + e_y e_x^T)).
   const double* pk; double MJ[16], MK[16];
   int nbf;
-  double cK, cLR, omega2; int use_lr;
+  double cK, cLR, omega, omega2; int use_lr;
   double* grad;                    // [natom][3]
   unsigned long long* counters;    // [3]: visited, computed, prim quartets
   const double* rys_tab;
@@ -69,6 +69,11 @@ __constant__ static uint16_t c_cart[4][10] = {
   {0x003, 0x012, 0x102, 0x021, 0x111, 0x201, 0x030, 0x120, 0x210, 0x300}};
 // per-component normalisation 1/sqrt((2lx-1)!!(2ly-1)!!(2lz-1)!!) (eq 38 "N"; O1)
 __host__ __device__ constexpr double dfact_odd(int n) { return n <= 0 ? 1.0 : (n == 1 ? 1.0 : (n == 2 ? 3.0 : 15.0)); }
+__host__ __device__ constexpr double cnorm_c(int l, int idx) {   // compile-time form (folds to an immediate after unrolling)
+  constexpr double r3 = 0.57735026918962576451, r15 = 0.25819888974716112568;
+  constexpr double t[4][10] = {{1.0}, {1.0, 1.0, 1.0}, {r3, 1.0, 1.0, r3, 1.0, r3}, {r15, r3, r3, r3, 1.0, r3, r15, r3, r3, r15}};
+  return t[l][idx];
+}
 __constant__ static double c_cnorm[4][10] = {
   {1.0},
   {1.0, 1.0, 1.0},

@@ -15,7 +15,7 @@
 #pragma once
 #include "tdg_common.cuh"
 #define TDG_NT (TDG_WARPS * TDG_WARP)
-#define TDG_ACC_DOUBLES (TDG_WARPS * (TDG_WARP + TDG_KB) * 6)
+#define TDG_ACC_DOUBLES ((TDG_WARPS * TDG_WARP + TDG_KB) * 6)   // per-warp bra slots + ket slots (each ket belongs to one warp)
 #ifndef TDG_RU_LIM
 #define TDG_RU_LIM 120
 #endif
@@ -46,7 +46,6 @@ struct QC {
   static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;
   static constexpr bool TWO_STAGE = SMALL && NROLE <= 2;   // measured: faster for 1-2 roles, slower for classes with more roles
-  static constexpr bool PREFETCH = false;   // software prefetch of the next quartet's blocks: measured SLOWER (L1 wavefront-bound), kept off
   static constexpr bool RYS_SH = NR <= 4;                                  // Rys table of this NR staged in shared memory
   static constexpr int RYS_SH_DOUBLES = RYS_SH ? rys_part_doubles(NR) : 0;
   static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
@@ -186,7 +185,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
             const double* v = vJL[b * ND + d]; const double* tt = tIL[a * ND + d]; const double* w = vKL[c * ND + d];
             const double gk = u.x * v[0] + u.y * v[1] + u.z * v[2] + u.w * v[3] + sv.x * tt[0] + sv.y * tt[1] + sv.z * tt[2] + sv.w * tt[3];
             const double gj = jv.x * w[0] + jv.y * w[1] + jv.z * w[2] + jv.w * w[3];
-            const double cn = deg * c_cnorm[LA][a] * c_cnorm[LB][b] * c_cnorm[LC][c] * c_cnorm[LD][d];
+            const double cn = deg * (cnorm_c(LA, a) * cnorm_c(LB, b) * cnorm_c(LC, c) * cnorm_c(LD, d));
             const int idx = ((ab - AB0) * NC + c) * ND + d;
             GF[idx] = cn * (gj + P.cK * gk);
             GL[idx] = cn * P.cLR * gk;
@@ -199,22 +198,23 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
   for (int t = 0; t < 9; ++t) g[t] = 0.0;
   const double ABx = bh.AB[0], ABy = bh.AB[1], ABz = bh.AB[2];
   const double CDx = kh.AB[0], CDy = kh.AB[1], CDz = kh.AB[2];
+  // primitive-pair record (tdg_common.cuh): p, Px, Py, Pz, K_ab/p, a, b, 1/p.  With rs = (p+q)^(-1/2):
+  //   2 pi^(5/2) K_ab K_cd / (p q sqrt(p+q)) = C (K_ab/p) (K_cd/q) rs;  1/(p+q) = rs^2;  s = omega (omega^2+rho)^(-1/2)  (S8)
   for (int ib = 0; ib < P.nppb; ++ib) {
     const d4 bp0 = ld256(bprim + ib * TDG_PRIM_STRIDE), bp1 = ld256(bprim + ib * TDG_PRIM_STRIDE + 4);
-    const double p = bp0.x, Px = bp0.y, Py = bp0.z, Pz = bp0.w, Kab = bp1.x, a2 = 2.0 * bp1.y, b2 = 2.0 * bp1.z;
+    const double p = bp0.x, Px = bp0.y, Py = bp0.z, Pz = bp0.w, Kab = 34.986836655249725693 /* 2 pi^(5/2) */ * bp1.x, a2 = 2.0 * bp1.y, b2 = 2.0 * bp1.z, rp = bp1.w;
     const double PAx = Px - bh.A[0], PAy = Py - bh.A[1], PAz = Pz - bh.A[2];
     for (int ik = 0; ik < P.nppk; ++ik) {
       const d4 kp0 = ld256(kprim + ik * TDG_PRIM_STRIDE), kp1 = ld256(kprim + ik * TDG_PRIM_STRIDE + 4);
-      const double q = kp0.x, Qx = kp0.y, Qy = kp0.z, Qz = kp0.w, Kcd = kp1.x, c2 = 2.0 * kp1.y;
+      const double q = kp0.x, Qx = kp0.y, Qy = kp0.z, Qz = kp0.w, c2 = 2.0 * kp1.y, rq = kp1.w;
       const double QCx = Qx - kh.A[0], QCy = Qy - kh.A[1], QCz = Qz - kh.A[2];
       const double PQx = Px - Qx, PQy = Py - Qy, PQz = Pz - Qz;
-      const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+      const double rs = rsqrt(p + q), rpq = rs * rs, rho = p * q * rpq;
       const double T = rho * (PQx * PQx + PQy * PQy + PQz * PQz);
-      const double pref = 34.986836655249725693 /* 2 pi^(5/2) */ * Kab * Kcd * rpq * sqrt(rpq) / rho;
-      const double rp = 1.0 / p, rq = 1.0 / q;
+      const double pref = Kab * kp1.x * rs;
       for (int op = 0; op <= P.use_lr; ++op) {
         double s2 = 1.0, ss = 1.0;
-        if (op == 1) { s2 = P.omega2 / (P.omega2 + rho); ss = sqrt(s2); }
+        if (op == 1) { ss = P.omega * rsqrt(P.omega2 + rho); s2 = ss * ss; }
         double xr[NR], wr[NR];
         rys_eval<NR>(rys, s2 * T, xr, wr);
         const double* __restrict__ G = op == 0 ? GF : GL;
@@ -330,61 +330,79 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
 
 __device__ __forceinline__ void red_add(double* addr, double v) { atomicAdd(addr, v); }
 
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-// Prefetch the six packed density blocks and the primitive-pair data of the NEXT survivor of this lane into L1 while
-// the current quartet is computed (the density gathers are the long-scoreboard stalls of the low-l classes).
-template <int LA, int LB, int LC, int LD>
-__device__ __forceinline__ void prefetch_quartet(const KParams& P, const PairHdr& bh, const PairHdr& kh, const double* bprim, const double* kprim) {
-  typedef QC<LA, LB, LC, LD> C;
-  const size_t n = (size_t)P.nbf;
-  const char* pk = reinterpret_cast<const char*>(P.pk);
-  const char* blk[6] = {pk + 32 * ((size_t)bh.offA * n + (size_t)C::NA * kh.offA), pk + 32 * ((size_t)bh.offB * n + (size_t)C::NB * kh.offB),
-                        pk + 32 * ((size_t)bh.offB * n + (size_t)C::NB * kh.offA), pk + 32 * ((size_t)bh.offA * n + (size_t)C::NA * kh.offB),
-                        pk + 32 * ((size_t)bh.offA * n + (size_t)C::NA * bh.offB), pk + 32 * ((size_t)kh.offA * n + (size_t)C::NC * kh.offB)};
-  constexpr int bytes[6] = {C::NA * C::NC * 32, C::NB * C::ND * 32, C::NB * C::NC * 32, C::NA * C::ND * 32, C::NA * C::NB * 32, C::NC * C::ND * 32};
-#pragma unroll
-  for (int q = 0; q < 6; ++q) {
-#pragma unroll
-    for (int o = 0; o < bytes[q]; o += 128) prefetch_l1(blk[q] + o);
-    if ((bytes[q] & 127) != 0 || bytes[q] > 128) prefetch_l1(blk[q] + bytes[q] - 32);   // last sector (blocks are only 32-byte aligned)
+// ---- step a4 (reading S9): one ket against the nb bras of the tile -> 32-bit survivor mask ----
+__device__ __forceinline__ unsigned screen_ket(const KParams& P, const PairHdr* s_bra, const double* s_dij, int nb, int bra0, int k,
+                                               const PairHdr& kh, bool dw, unsigned long long& n_vis, unsigned long long& n_cmp) {
+  const int ns = P.nshell;
+  const int ksh = kh.ish, lsh = kh.jsh;
+  const double Qk = kh.Q;
+  const double dkl = dw ? __ldg(P.dmax + (size_t)ksh * ns + lsh) : 0.0;
+  const bool ket_one = kh.atomA == kh.atomB;
+  unsigned mask = 0;
+  for (int b = 0; b < nb; ++b) {
+    if (P.same_bucket && k > bra0 + b) continue;
+    const PairHdr& bh = s_bra[b];
+    if (P.tau > 0.0) {
+      const double qq = bh.Q * Qk;
+      if (!(qq >= P.tau)) continue;
+      ++n_vis;
+      if (dw && qq * (P.CJ * s_dij[b] * dkl) < P.tau) {
+        // W = max(W_J, W_K) (S9): the J-type bound alone does not keep the quartet, so gather the four K-type maxima
+        const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + ksh), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + lsh);
+        const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + lsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + ksh);
+        const double x1 = dik * djl, x2 = dil * djk;
+        if (qq * (P.CK * (x1 > x2 ? x1 : x2)) < P.tau) continue;
+      }
+    } else ++n_vis;
+    if (!tdg_sample_keep(bh.ish, bh.jsh, ksh, lsh, P.sample_mod, P.sample_seed)) continue;
+    ++n_cmp;
+    // all four shells on one atom: the four centre derivatives sum to zero on that atom (reading S11)
+    if (ket_one && bh.atomA == bh.atomB && bh.atomA == kh.atomA) continue;
+    mask |= 1u << b;
   }
-  prefetch_l1(bprim); prefetch_l1(kprim);
+  return mask;
+}
+
+// Survivor s of a warp's list (ket-major: lane o owns ket o with survivor mask `mask` and exclusive prefix `pre`):
+// owner lane = largest o with pre_o <= s; bra = position of the (s - pre_o + 1)-th set bit of its mask.
+__device__ __forceinline__ void warp_survivor(unsigned mask, int pre, int s, int& o, int& b) {
+  o = 0;
+#pragma unroll
+  for (int step = 16; step > 0; step >>= 1) { const int pv = __shfl_sync(0xffffffffu, pre, o + step); if (pv <= s) o += step; }
+  const unsigned m = __shfl_sync(0xffffffffu, mask, o);
+  const int r = s - __shfl_sync(0xffffffffu, pre, o);
+  b = (int)__fns(m, 0, r + 1);
 }
 
 // Phase 2 of the kernel for one role (slice [AB0, AB0+ABC) of the bra function pairs).
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
-__device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
-                                                  const uint16_t* s_list, double* s_gb, double* s_gk, int total, int bra0, int k0, const double* __restrict__ rys) {
-  // Each warp takes passes of 32 consecutive entries of the ket-major survivor list.  Gradient accumulation uses no
-  // atomics (shared-memory FP64 atomics are CAS loops of ~60 iterations per warp and 6 RED per quartet saturate L2;
-  // both measured): lanes with the same ket are contiguous, so the ket-centre terms are summed by a segmented warp
-  // shuffle scan and added by the segment head to this warp's private slot; the bra-centre terms are added to this
-  // warp's private slots segment by segment (bras are distinct within a segment).  Fourth centre: eq 41.
-  typedef QC<LA, LB, LC, LD> C0;
+__device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket, unsigned mask, int pre, int tot,
+                                                  double* s_gb, double* s_gk, int bra0, int k0, const double* __restrict__ rys) {
+  // Each warp owns the 32 kets [32 w, 32 w + 32) of the chunk and takes passes of 32 consecutive entries of its ket-major
+  // survivor list.  Gradient accumulation uses no atomics (shared-memory FP64 atomics are CAS loops of ~60 iterations
+  // per warp and 6 RED per quartet saturate L2; both measured): lanes with the same ket are contiguous, so the ket-centre
+  // terms are summed by a segmented warp shuffle scan and added by the segment head to the ket's slot (only this warp
+  // touches it); the bra-centre terms are added to this warp's private bra slots segment by segment (bras are distinct
+  // within a segment).  Fourth centre: eq 41.
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double* my_gb = s_gb + warp * (TDG_WARP * 6);
-  double* my_gk = s_gk + warp * (TDG_KB * 6);
-  for (int base = warp * TDG_WARP; base < total; base += TDG_NT) {
+  double* my_gk = s_gk + warp * (TDG_KW * 6);
+  const int kw0 = warp * TDG_KW;
+  for (int base = 0; base < tot; base += TDG_WARP) {
     const int s = base + lane;
-    const bool act = s < total;
-    const unsigned e = act ? s_list[s] : 0u;
-    const int kt = e >> 5, b = e & 31;
-    if (C0::PREFETCH && s + TDG_NT < total) {
-      const unsigned e2 = s_list[s + TDG_NT];
-      const int kt2 = e2 >> 5, b2 = e2 & 31;
-      prefetch_quartet<LA, LB, LC, LD>(P, s_bra[b2], s_ket[kt2], P.bra_prim + (size_t)(bra0 + b2) * P.nppb * TDG_PRIM_STRIDE,
-                                       P.ket_prim + (size_t)(k0 + kt2) * P.nppk * TDG_PRIM_STRIDE);
-    }
+    const bool act = s < tot;
+    int kt, b;
+    warp_survivor(mask, pre, act ? s : tot - 1, kt, b);
     double g[9];
     if (act) {
       const PairHdr& bh = s_bra[b];
-      const PairHdr& kh = s_ket[kt];
+      const PairHdr& kh = s_ket[kw0 + kt];
       double deg = 1.0;
       if (bh.ish == bh.jsh) deg *= 0.5;
       if (kh.ish == kh.jsh) deg *= 0.5;
-      if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
+      if (P.same_bucket && k0 + kw0 + kt == bra0 + b) deg *= 0.5;
       quartet_grad<LA, LB, LC, LD, AB0, ABC>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
-                                             P.ket_prim + (size_t)(k0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys, g);
+                                             P.ket_prim + (size_t)(k0 + kw0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys, g);
     } else {
 #pragma unroll
       for (int x = 0; x < 9; ++x) g[x] = 0.0;
@@ -420,52 +438,53 @@ __device__ __forceinline__ void process_survivors(const KParams& P, const PairHd
 template <int LA, int LB, int LC, int LD, int R>
 struct RoleDispatch {
   typedef QC<LA, LB, LC, LD> C;
-  static __device__ __forceinline__ void run(int role, const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket,
-                                             const uint16_t* s_list, double* s_gb, double* s_gk, int total, int bra0, int k0, const double* __restrict__ rys) {
+  static __device__ __forceinline__ void run(int role, const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket, unsigned mask, int pre, int tot,
+                                             double* s_gb, double* s_gk, int bra0, int k0, const double* __restrict__ rys) {
     if constexpr (R < C::NROLE) {
       constexpr int AB0 = R * C::ABN;
       constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
-      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, s_list, s_gb, s_gk, total, bra0, k0, rys);
-      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, s_list, s_gb, s_gk, total, bra0, k0, rys);
+      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, mask, pre, tot, s_gb, s_gk, bra0, k0, rys);
+      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, mask, pre, tot, s_gb, s_gk, bra0, k0, rys);
     }
   }
 };
 
+// Block work item -> (bra tile, ket chunk): largest t with cum[t] <= item.
+__device__ __forceinline__ void find_work_item(const KParams& P, int item, int& tile, int& chunk) {
+  int lo = 0, hi = P.ntiles;
+  while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (__ldg(P.cum + mid) <= item) lo = mid; else hi = mid; }
+  tile = lo; chunk = item - __ldg(P.cum + lo);
+}
 
-
+#ifndef TDG_MINB
+#define TDG_MINB 1
+#endif
 template <int LA, int LB, int LC, int LD>
-__global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant__ KParams P) {
+__global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid_constant__ KParams P) {
   __shared__ PairHdr s_bra[TDG_WARP];
   __shared__ PairHdr s_ket[TDG_KB];
   __shared__ double s_dij[TDG_WARP];
-  __shared__ uint16_t s_list[TDG_WARP * TDG_KB];      // surviving quartets of this work item: ket_local << 5 | bra_local
-  __shared__ int s_wcnt[TDG_WARPS];
-  // dynamic shared memory: per-warp private accumulators, then the Rys table of this class (QC::RYS_SH)
+  // dynamic shared memory: accumulators (per-warp bra slots, then the ket slots), then the Rys table of this class (QC::RYS_SH)
   extern __shared__ double2 s_dyn[];
   typedef QC<LA, LB, LC, LD> C;
   double* s_gb = reinterpret_cast<double*>(s_dyn);            // [warp][bra][centre A,B][xyz]
-  double* s_gk = s_gb + TDG_WARPS * TDG_WARP * 6;             // [warp][ket][centre C,D][xyz]
+  double* s_gk = s_gb + TDG_WARPS * TDG_WARP * 6;             // [ket][centre C,D][xyz]; ket 32 w + o belongs to warp w
   double2* s_rys = s_dyn + TDG_ACC_DOUBLES / 2;
-  // block work item -> (bra tile, ket chunk): largest t with cum[t] <= item
-  const int item = blockIdx.x;
-  int lo = 0, hi = P.ntiles;
-  while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (__ldg(P.cum + mid) <= item) lo = mid; else hi = mid; }
-  const int tile = lo, chunk = item - __ldg(P.cum + tile);
-  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-  const int ns = P.nshell;
+  int tile, chunk;
+  find_work_item(P, blockIdx.x, tile, chunk);
+  const int t = threadIdx.x, lane = t & 31;
   const int bra0 = tile * TDG_WARP, k0 = chunk * TDG_KB;
   const int nb = min(TDG_WARP, P.nbra - bra0);
   const bool dw = P.tau > 0.0 && P.density_weighted;
   if (t < nb) {
     const PairHdr h = P.bra_hdr[bra0 + t];
     s_bra[t] = h;
-    s_dij[t] = dw ? __ldg(P.dmax + (size_t)h.ish * ns + h.jsh) : 0.0;
+    s_dij[t] = dw ? __ldg(P.dmax + (size_t)h.ish * P.nshell + h.jsh) : 0.0;
   }
   const int k = k0 + t;
   const bool ket_ok = k < P.nket;
   if (ket_ok) s_ket[t] = P.ket_hdr[k];
-  for (int i = t; i < TDG_WARPS * TDG_WARP * 6; i += TDG_NT) s_gb[i] = 0.0;
-  for (int i = t; i < TDG_WARPS * TDG_KB * 6; i += TDG_NT) s_gk[i] = 0.0;
+  for (int i = t; i < TDG_ACC_DOUBLES; i += TDG_NT) s_gb[i] = 0.0;
   const double* rys = P.rys_tab + rys_part_off(C::NR);
   if (C::RYS_SH) {
     const double2* src = reinterpret_cast<const double2*>(rys);
@@ -473,53 +492,18 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
     rys = reinterpret_cast<const double*>(s_rys);
   }
   __syncthreads();
-  // ---- phase 1 (step a4; reading S9): one ket per thread, test it against the 32 bras ----
-  unsigned mask = 0;
+  // ---- phase 1 (step a4): one ket per thread, tested against the 32 bras; warp scan of the survivor counts ----
   unsigned long long n_vis = 0, n_cmp = 0;
-  if (ket_ok) {
-    const PairHdr& kh = s_ket[t];
-    const int ksh = kh.ish, lsh = kh.jsh;
-    const double Qk = kh.Q;
-    const double dkl = dw ? __ldg(P.dmax + (size_t)ksh * ns + lsh) : 0.0;
-    const bool ket_one = kh.atomA == kh.atomB;
-    for (int b = 0; b < nb; ++b) {
-      if (P.same_bucket && k > bra0 + b) continue;
-      const PairHdr& bh = s_bra[b];
-      if (P.tau > 0.0) {
-        const double qq = bh.Q * Qk;
-        if (!(qq >= P.tau)) continue;
-        ++n_vis;
-        if (dw && qq * (P.CJ * s_dij[b] * dkl) < P.tau) {
-          // W = max(W_J, W_K) (S9): the J-type bound alone does not keep the quartet, so gather the four K-type maxima
-          const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + ksh), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + lsh);
-          const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + lsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + ksh);
-          const double x1 = dik * djl, x2 = dil * djk;
-          if (qq * (P.CK * (x1 > x2 ? x1 : x2)) < P.tau) continue;
-        }
-      } else ++n_vis;
-      if (!tdg_sample_keep(bh.ish, bh.jsh, ksh, lsh, P.sample_mod, P.sample_seed)) continue;
-      ++n_cmp;
-      // all four shells on one atom: the four centre derivatives sum to zero on that atom (reading S11)
-      if (ket_one && bh.atomA == bh.atomB && bh.atomA == kh.atomA) continue;
-      mask |= 1u << b;
-    }
-  }
-  // block-wide exclusive scan of the survivor counts -> compacted list, ket-major
+  const unsigned mask = ket_ok ? screen_ket(P, s_bra, s_dij, nb, bra0, k, s_ket[t], dw, n_vis, n_cmp) : 0u;
   const int cnt = __popc(mask);
   int incl = cnt;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-  if (lane == 31) s_wcnt[warp] = incl;
+  const int tot = __shfl_sync(0xffffffffu, incl, 31);
+  // ---- phase 2 (steps a5-a8): each warp processes the survivors of its own 32 kets densely, one quartet per thread per pass ----
+  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, mask, incl - cnt, tot, s_gb, s_gk, bra0, k0, rys);
   __syncthreads();
-  int off = incl - cnt, total = 0;
-#pragma unroll
-  for (int w = 0; w < TDG_WARPS; ++w) { const int c = s_wcnt[w]; if (w < warp) off += c; total += c; }
-  while (mask) { const int b = __ffs(mask) - 1; mask &= mask - 1; s_list[off++] = (uint16_t)((t << 5) | b); }
-  __syncthreads();
-  // ---- phase 2 (steps a5-a8): survivors are processed densely, one quartet per thread per pass ----
-  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, s_list, s_gb, s_gk, total, bra0, k0, rys);
-  __syncthreads();
-  // flush: sum the warps' private slots, one FP64 RED per touched (pair, centre, xyz)
+  // flush: sum the warps' private bra slots, one FP64 RED per touched (pair, centre, xyz)
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
     double v = 0.0;
     const PairHdr* h;
@@ -530,8 +514,7 @@ __global__ void __launch_bounds__(TDG_NT) tdg_grad_kernel(const __grid_constant_
       h = s_bra + i / 6; r = i % 6;
     } else {
       const int ii = i - TDG_WARP * 6;
-#pragma unroll
-      for (int w = 0; w < TDG_WARPS; ++w) v += s_gk[w * (TDG_KB * 6) + ii];
+      v = s_gk[ii];
       h = s_ket + ii / 6; r = ii % 6;
     }
     if (v != 0.0) red_add(P.grad + 3 * (r < 3 ? h->atomA : h->atomB) + (r < 3 ? r : r - 3), v);

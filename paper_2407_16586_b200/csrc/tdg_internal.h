@@ -12,10 +12,9 @@ cudaError_t tdg_launch_schwarz(const DevShell* sh, int ns, const double* xyz, co
                                const double* rys_tab, double* Q, cudaStream_t s);
 // out = max |M - M^T|  (device scalar, must be zeroed)
 cudaError_t tdg_launch_asym(const double* M, int n, double* out, cudaStream_t s);
-// S = (M + M^T)/2, N = (M - M^T)/2
-cudaError_t tdg_launch_symsplit(const double* M, int n, double* S, double* N, cudaStream_t s);
 // m[i*ns+j] = max over the nmat matrices and the block (i,j) of max(|M_mn|, |M_nm|)   (reading S9: d_ij)
-cudaError_t tdg_launch_dmax(const double* const* mats_dev, int nmat, int n, const DevShell* sh, int ns, double* m, cudaStream_t s);
+struct MatList { const double* m[16]; int n; };   // passed to the kernel by value: no upload, no host synchronisation
+cudaError_t tdg_launch_dmax(const MatList& mats, int n, const DevShell* sh, int ns, double* m, cudaStream_t s);
 cudaError_t tdg_launch_rys(int n, int count, const double* T, const double* rho, double omega, const double* tab, double* out, cudaStream_t s);
 cudaError_t tdg_run_fp64_peak(double ms, double* tflops);
 

@@ -2,11 +2,13 @@
 
     python -m paper_2407_16586_b200.profile_run [config=3] [calls=1]
 """
+import json
+import os
 import sys
 
 import torch
 
-from paper_2407_16586_b200 import tdgrad
+from paper_2407_16586_b200 import ncu_classes, tdgrad
 from paper_2407_16586_b200 import workload as wl
 
 
@@ -22,6 +24,12 @@ def main():
     for _ in range(calls):
         g, st = ctx.gradient(pairs, wJ, wK, wl.C_J, wl.C_K, wl.C_LR, wl.OMEGA)
     print("quartets", st["quartets_computed"], "ms", st["ms_total"])
+    os.makedirs("gpurun_out", exist_ok=True)    # per-class counts of the profiled call, merged into the summary by ncu_classes.py
+    with open(os.path.join("gpurun_out", "profile_run_cfg%d.json" % cfg), "w") as fh:
+        json.dump(dict(config=cfg, source_hash=ncu_classes.source_hash(), quartets=st["quartets_computed"], ms_total=st["ms_total"],
+                       quartets_by_class={tdgrad.class_name(c): st["quartets_by_class"][c] for c in range(tdgrad.NCLASS) if st["quartets_by_class"][c]},
+                       prim_quartets_by_class={tdgrad.class_name(c): st["prim_quartets_by_class"][c] for c in range(tdgrad.NCLASS) if st["quartets_by_class"][c]},
+                       ms_by_class={tdgrad.class_name(c): st["ms_by_class"][c] for c in range(tdgrad.NCLASS) if st["quartets_by_class"][c]}), fh)
     ctx.close()
 
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libtdgrad.so")
 NCLASS = 55
 _lib = None
 
-SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_shard", "tdg_plan", "tdg_schwarz", "tdg_gradient",
+SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_shard", "tdg_set_streams", "tdg_plan", "tdg_schwarz", "tdg_gradient",
            "tdg_energy", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
 
 
@@ -32,11 +32,12 @@ class Stats(C.Structure):
     _fields_ = [("pairs_total", C.c_int64), ("pairs_kept", C.c_int64), ("quartets_visited", C.c_int64),
                 ("quartets_computed", C.c_int64), ("prim_quartets", C.c_int64), ("quartets_by_class", C.c_int64 * NCLASS),
                 ("prim_quartets_by_class", C.c_int64 * NCLASS),
-                ("ms_by_class", C.c_float * NCLASS), ("ms_prepare", C.c_float), ("ms_total", C.c_float), ("launches", C.c_int32)]
+                ("ms_by_class", C.c_float * NCLASS), ("ms_prepare", C.c_float), ("ms_total", C.c_float), ("launches", C.c_int32),
+                ("groups", C.c_int32)]
 
     def asdict(self):
         d = {k: getattr(self, k) for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets",
-                                           "ms_prepare", "ms_total", "launches")}
+                                           "ms_prepare", "ms_total", "launches", "groups")}
         d["quartets_by_class"] = list(self.quartets_by_class)
         d["prim_quartets_by_class"] = list(self.prim_quartets_by_class)
         d["ms_by_class"] = list(self.ms_by_class)
@@ -158,6 +159,10 @@ class Context:
     def set_shard(self, rank: int, nranks: int):
         """This context computes the work items `rank` mod `nranks`; call before :meth:`plan`."""
         self._check(lib().tdg_set_shard(self._h, C.c_int(rank), C.c_int(nranks)), "tdg_set_shard")
+
+    def set_streams(self, nstreams: int):
+        """Deal the class launches of a call over `nstreams` CUDA streams (the caller's + internal ones)."""
+        self._check(lib().tdg_set_streams(self._h, C.c_int(nstreams)), "tdg_set_streams")
 
     def plan(self, tau=0.0, density_weighted=0, sample_mod=0, sample_seed=0):
         opt = Options(tau, density_weighted, sample_mod, sample_seed)

@@ -230,6 +230,7 @@ def make_densities_torch(nbf: int, seed: int, device, n_occ: int | None = None):
     co = co * torch.sign(torch.diagonal(r))
     del r
     D = co @ co.T
+    D = 0.5 * (D + D.T)      # exactly symmetric whatever the GEMM's summation order (a rounding-level antisymmetric part would take a matrix slot)
     P = torch.randn((nbf, nbf), generator=g, dtype=f64, device=device)
     P = 0.5 * (P + P.T)
     P *= float(np.sqrt(n_occ)) / torch.linalg.norm(P)

@@ -14,6 +14,15 @@ def tiny_system(with_f=False, tau=0.0):
     return wl.make_custom_system(xyz, [a0, a1, a2], tau=tau)
 
 
+def two_centre_spdf_system(tau=0.0):
+    """Two atoms, each with s, p, d and f shells (two with 2 primitives): every one of the 55 quartet classes occurs,
+    (ff|ff) included with shells on different centres."""
+    xyz = np.array([[0.0, 0.0, 0.0], [1.1, -0.7, 0.9]])
+    a0 = [(0, [2.3, 0.6], [0.5, 0.6]), (1, [1.1], [1.0]), (2, [0.9], [1.0]), (3, [1.3, 0.5], [0.4, 0.7])]
+    a1 = [(0, [0.7], [1.0]), (1, [1.9, 0.5], [0.3, 0.8]), (2, [1.4], [1.0]), (3, [0.8], [1.0])]
+    return wl.make_custom_system(xyz, [a0, a1], tau=tau)
+
+
 def densities(nbf, seed=7, n_occ=None):
     return wl.make_densities(nbf, np.random.SeedSequence(seed), n_occ=n_occ)
 

@@ -44,8 +44,8 @@ def test_binding_lists_every_declared_symbol():
 def test_stats_struct_matches_header():
     from paper_2407_16586_b200 import tdgrad
 
-    # 5 int64 + 2*55 int64 + 55 float + 2 float + int32, padded to 8
-    raw = 8 * 5 + 8 * 55 * 2 + 4 * 55 + 4 * 2 + 4
+    # 5 int64 + 2*55 int64 + 55 float + 2 float + 2 int32, padded to 8
+    raw = 8 * 5 + 8 * 55 * 2 + 4 * 55 + 4 * 2 + 4 * 2
     assert C.sizeof(tdgrad.Stats) == (raw + 7) // 8 * 8
     assert C.sizeof(tdgrad.Options) == 24
 

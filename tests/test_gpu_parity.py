@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from paper_2407_16586_b200 import workload as wl
-from tests.helpers import CALL, densities, tiny_system
+from tests.helpers import CALL, densities, tiny_system, two_centre_spdf_system
 
 pytestmark = pytest.mark.gpu
 
@@ -88,6 +88,25 @@ def test_tiny_system_all_classes(ctx, orc, with_f):
         assert st[k] == rst[k], k
 
 
+def test_two_centre_spdf_every_class_in_full(ctx, orc):
+    """All 55 quartet classes, f shells on both centres, no screening, no subsample: every class kernel is compared on
+    real two-centre quartets (the single f shell of tiny_system only gives the one-atom (ff|ff) the kernel skips)."""
+    s = two_centre_spdf_system()
+    D, P, T = densities(s.nbf, seed=13)
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK)
+    _compare(g, ref)
+    for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets"):
+        assert st[k] == rst[k], k
+    assert all(c > 0 for c in st["quartets_by_class"]), st["quartets_by_class"]
+    # nonsymmetric pairs through the same classes
+    rng = np.random.default_rng(8)
+    M = [rng.standard_normal((s.nbf, s.nbf)) for _ in range(3)]
+    pairs2 = [(M[0], M[1]), (M[2], M[2])]
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs2, np.array([0.9, -0.4]), np.array([0.6, 1.2]))
+    _compare(g, ref)
+
+
 def test_tiny_general_pairs_and_weights(ctx, orc):
     """Arbitrary nonsymmetric A != B pairs and weights exercise the sym/antisym split of the K term."""
     s = tiny_system(with_f=False)
@@ -153,6 +172,7 @@ def test_cfg2_f_shells_subsample(ctx, orc):
     assert st["pairs_kept"] == rst["pairs_kept"]
     assert st["quartets_visited"] == rst["quartets_visited"]
     assert st["quartets_computed"] == rst["quartets_computed"]
+    assert all(c > 0 for c in st["quartets_by_class"]), st["quartets_by_class"]   # the subsample hits all 55 classes
 
 
 @pytest.mark.slow
@@ -214,22 +234,6 @@ def test_gpu_gradient_is_derivative_of_gpu_energy(ctx):
         assert abs(fd - g[atom, x]) <= 1e-6, (atom, x, fd, g[atom, x])
 
 
-@pytest.mark.slow
-@pytest.mark.skipif(os.environ.get("TDG_RUN_CFG4") != "1", reason="several minutes of CPU oracle time; set TDG_RUN_CFG4=1 (result of the round-1 run: profiles/r01_cfg4_parity.md)")
-def test_cfg4_subsample_largest_configuration(ctx, orc):
-    """1024 waters (25 600 bf, 21 GB packed densities): deterministic subsample both sides evaluate (S12)."""
-    s = wl.make_system(4)
-    D, P, T = wl.make_densities(s.nbf, wl.density_seed(4))
-    pairs, wJ, wK = wl.default_call(D, P, T)
-    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, sample_mod=4000000, sample_seed=4)
-    d = float(np.max(np.abs(g - ref)))
-    print("cfg4 subsample: quartets gpu/oracle", st["quartets_computed"], rst["quartets_computed"], "pairs_kept", st["pairs_kept"], rst["pairs_kept"],
-          "max|dg|", d, "max|g|", float(np.max(np.abs(ref))))
-    _compare(g, ref)
-    assert st["pairs_kept"] == rst["pairs_kept"]
-    assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 3
-
-
 @pytest.mark.parametrize("nranks", [2, 3])
 def test_sharded_work_items_partition_the_gradient(ctx, orc, nranks):
     """SURVEY.md 8(e) / PAPER.md:309: the rank shards (tdg_set_shard) partition the quartets exactly (integer counts add up
@@ -269,3 +273,19 @@ def test_set_shard_rejects_bad_arguments(ctx):
         with pytest.raises(tdgrad.TdgError):
             ctx.set_shard(rank, n)
     ctx.set_shard(0, 1)
+
+
+@pytest.mark.slow
+def test_cfg4_subsample_largest_configuration(ctx, orc):
+    """1024 waters (25 600 bf, 21 GB packed densities): deterministic subsample both sides evaluate (S12).
+    Last in the file: ~12 min, almost all of it the oracle's own Schwarz bounds over 7.5e7 shell pairs."""
+    s = wl.make_system(4)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(4))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, sample_mod=4000000, sample_seed=4)
+    d = float(np.max(np.abs(g - ref)))
+    print("cfg4 subsample: quartets gpu/oracle", st["quartets_computed"], rst["quartets_computed"], "pairs_kept", st["pairs_kept"], rst["pairs_kept"],
+          "max|dg|", d, "max|g|", float(np.max(np.abs(ref))))
+    _compare(g, ref)
+    assert st["pairs_kept"] == rst["pairs_kept"]
+    assert abs(st["quartets_computed"] - rst["quartets_computed"]) <= 3
