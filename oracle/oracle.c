@@ -739,6 +739,175 @@ int orc_gradient_n4(SYS_ARGS, int npair, const double *const *A, const double *c
     return 0;
 }
 
+/* ---------------------------------------------------------------- NEXT-1: Fock-type (J/K) build
+ * PAPER.md:138 (eq 19), PAPER.md:197-207 (eqs 33-34).  For each input matrix B_k (general, nonsymmetric allowed):
+ *
+ *   F_k[mn] = sum_{ls} [ wJ_k B_k[sl] (mn|ls)  -  X_k[sl] ( cK (ml|sn) + cLR (ml|sn)_lr ) ],   X_k = wK_k B_k + wKT_k B_k^T
+ *
+ * Eq 34 is wJ = 4, wK = wKT = 1, cK = alpha, cLR = beta  ((ms|ln) with B[sl] is (ml|sn) with B^T[sl]);
+ * eq 19 is wJ = 2, wK = 1, wKT = 0.  The XC kernel term of both equations is out of scope.
+ *
+ * orc_fock_n4: the definition, all nshell^4 shell quartets, no symmetry, no screening (tiny inputs). */
+int orc_fock_n4(SYS_ARGS, int nmat, const double *const *B, const double *wJ, const double *wK, const double *wKT,
+                double cK, double cLR, double omega, double *const *F) {
+    sys_t s; int rc = sys_init(&s, SYS_PASS); if (rc) return rc;
+    size_t n = (size_t)s.nbf;
+    work_t *w = work_new();
+    for (int q = 0; q < nmat; ++q) memset(F[q], 0, sizeof(double) * n * n);
+    for (int i = 0; i < nshell; ++i) for (int j = 0; j < nshell; ++j)
+    for (int k = 0; k < nshell; ++k) for (int l = 0; l < nshell; ++l) {
+        shell_quartet(&s, i, j, k, l, 0.0, w, w->val, NULL);
+        if (cLR != 0.0) shell_quartet(&s, i, j, k, l, omega, w, w->val2, NULL);
+        int ni = s.off[i + 1] - s.off[i], nj = s.off[j + 1] - s.off[j];
+        int nk = s.off[k + 1] - s.off[k], nl = s.off[l + 1] - s.off[l];
+        for (int a = 0; a < ni; ++a) for (int b = 0; b < nj; ++b)
+        for (int c = 0; c < nk; ++c) for (int d = 0; d < nl; ++d) {
+            size_t p_ = s.off[i] + a, q_ = s.off[j] + b, r_ = s.off[k] + c, s_ = s.off[l] + d;
+            size_t idx = (((size_t)a * nj + b) * nk + c) * nl + d;
+            double v = w->val[idx], vk = cK * v + (cLR != 0.0 ? cLR * w->val2[idx] : 0.0);
+            for (int m = 0; m < nmat; ++m) {
+                /* Coulomb: this integral read as (mn|ls) = (pq|rs):  F[pq] += wJ B[sr] (pq|rs) */
+                F[m][p_ * n + q_] += wJ[m] * B[m][s_ * n + r_] * v;
+                /* exchange: this integral read as (ml|sn) = (pq|rs): m=p, l=q, s=r, n=s:  F[ps] -= X[s l] = X[r q] */
+                F[m][p_ * n + s_] -= (wK[m] * B[m][r_ * n + q_] + wKT[m] * B[m][q_ * n + r_]) * vk;
+            }
+        }
+    }
+    work_free(w); sys_free(&s);
+    return 0;
+}
+
+/* Production loop: unique shell quartets i>=j, k>=l, ij>=kl with degeneracy deg, every integral digested into the
+ * blocks its 8 index permutations touch:
+ *   J:  F[mn] += wJ (B[ls]+B[sl]) I,  F[nm] += same,  F[ls] += wJ (B[mn]+B[nm]) I,  F[sl] += same
+ *   K:  F[ms] -= X[ln] Ik, F[ns] -= X[lm] Ik, F[ml] -= X[sn] Ik, F[nl] -= X[sm] Ik,
+ *       F[ln] -= X[ms] Ik, F[sn] -= X[ml] Ik, F[lm] -= X[ns] Ik, F[sm] -= X[nl] Ik        (Ik = cK I + cLR I_lr)
+ * Screening: pair kept iff tau<=0 or Q_ij Q_max >= tau; quartet kept iff Q_ij Q_kl >= tau and (if density_weighted)
+ *   Q_ij Q_kl W >= tau,  W = max( CJ max(d_ij, d_kl), CK max(d_ik, d_il, d_jk, d_jl) ),  d = block maxima over all B_k (both
+ *   orientations), CJ = max_k |wJ_k|, CK = (|cK|+|cLR|) max_k (|wK_k|+|wKT_k|)   ("the product of the density
+ *   matrix B_k and the Schwarz upper bound ... used as the screening parameter").  Subsample rule S12. */
+int orc_fock(SYS_ARGS, const orc_options *opt, int nmat, const double *const *B, const double *wJ, const double *wK,
+             const double *wKT, double cK, double cLR, double omega, double *const *F, orc_stats *st) {
+    sys_t s; int rc = sys_init(&s, SYS_PASS); if (rc) return rc;
+    if (cLR != 0.0 && omega <= 0.0) { sys_free(&s); return -3; }
+    int ns = nshell; size_t n = (size_t)s.nbf;
+    double tau = opt ? opt->tau : 0.0;
+    int dw = opt ? opt->density_weighted : 0;
+    uint32_t smod = opt ? opt->sample_mod : 0, sseed = opt ? opt->sample_seed : 0;
+    double *Q = NULL, *dm = NULL;
+    double CJ = 0.0, CK = 0.0;
+    for (int m = 0; m < nmat; ++m) {
+        if (fabs(wJ[m]) > CJ) CJ = fabs(wJ[m]);
+        if (fabs(wK[m]) + fabs(wKT[m]) > CK) CK = fabs(wK[m]) + fabs(wKT[m]);
+    }
+    CK *= fabs(cK) + fabs(cLR);
+    size_t np_all = (size_t)ns * (ns + 1) / 2;
+    pair_t *pairs = (pair_t *)malloc(sizeof(pair_t) * np_all);
+    size_t npk = 0;
+    if (tau > 0.0) {
+        Q = (double *)malloc(sizeof(double) * (size_t)ns * ns);
+        schwarz_all(&s, Q);
+        double Qmax = 0.0;
+        for (size_t t = 0; t < (size_t)ns * ns; ++t) if (Q[t] > Qmax) Qmax = Q[t];
+        for (int i = 0; i < ns; ++i) for (int j = 0; j <= i; ++j)
+            if (Q[(size_t)i * ns + j] * Qmax >= tau) { pairs[npk].i = i; pairs[npk].j = j; pairs[npk].Q = Q[(size_t)i * ns + j]; ++npk; }
+        if (dw) {
+            dm = (double *)malloc(sizeof(double) * (size_t)ns * ns);
+            density_maxima(&s, nmat, B, dm);
+        }
+        qsort(pairs, npk, sizeof(pair_t), pair_cmp);
+    } else {
+        for (int i = 0; i < ns; ++i) for (int j = 0; j <= i; ++j) { pairs[npk].i = i; pairs[npk].j = j; pairs[npk].Q = 1.0; ++npk; }
+    }
+    int nthr = 1;
+#ifdef _OPENMP
+    nthr = omp_get_max_threads();
+#endif
+    size_t nout = n * n * (size_t)nmat;
+    /* per-thread copies summed in a fixed order when they fit in ~1.6 GB, else one copy updated with atomic adds */
+    int shared = nout * (size_t)nthr > ((size_t)1 << 27) * (size_t)(nthr > 1);
+    double *acc = (double *)calloc(shared ? nout : nout * (size_t)nthr, sizeof(double));
+    if (!acc) { free(pairs); free(Q); free(dm); sys_free(&s); return -4; }
+    int64_t visited = 0, computed = 0, primq = 0;
+    int use_lr = (cLR != 0.0);
+#pragma omp parallel reduction(+ : visited, computed, primq)
+    {
+        int tid = 0;
+#ifdef _OPENMP
+        tid = omp_get_thread_num();
+#endif
+        double *Ft = shared ? acc : acc + nout * (size_t)tid;
+        work_t *w = work_new();
+#pragma omp for schedule(dynamic, 1)
+        for (long pa = 0; pa < (long)npk; ++pa) {
+            int i = pairs[pa].i, j = pairs[pa].j;
+            double Qij = pairs[pa].Q;
+            for (long pb = 0; pb <= pa; ++pb) {
+                int k = pairs[pb].i, l = pairs[pb].j;
+                if (tau > 0.0) {
+                    double qq = Qij * pairs[pb].Q;
+                    if (qq < tau) break;
+                    ++visited;
+                    if (dw) {
+                        double dij = dm[(size_t)i * ns + j], dkl = dm[(size_t)k * ns + l];
+                        double dik = dm[(size_t)i * ns + k], djl = dm[(size_t)j * ns + l];
+                        double dil = dm[(size_t)i * ns + l], djk = dm[(size_t)j * ns + k];
+                        double mj = dij > dkl ? dij : dkl;
+                        double mk = dik; if (djl > mk) mk = djl; if (dil > mk) mk = dil; if (djk > mk) mk = djk;
+                        double W = CJ * mj, WK = CK * mk;
+                        if (WK > W) W = WK;
+                        if (qq * W < tau) continue;
+                    }
+                } else ++visited;
+                if (!sample_keep(i, j, k, l, smod, sseed)) continue;
+                ++computed;
+                double deg = 1.0;
+                if (i == j) deg *= 0.5;
+                if (k == l) deg *= 0.5;
+                if (i == k && j == l) deg *= 0.5;
+                primq += shell_quartet(&s, i, j, k, l, 0.0, w, w->val, NULL);
+                if (use_lr) shell_quartet(&s, i, j, k, l, omega, w, w->val2, NULL);
+                int ni = s.off[i + 1] - s.off[i], nj = s.off[j + 1] - s.off[j];
+                int nk = s.off[k + 1] - s.off[k], nl = s.off[l + 1] - s.off[l];
+                for (int a = 0; a < ni; ++a) for (int b = 0; b < nj; ++b)
+                for (int c = 0; c < nk; ++c) for (int d = 0; d < nl; ++d) {
+                    size_t m_ = s.off[i] + a, n_ = s.off[j] + b, l_ = s.off[k] + c, s_ = s.off[l] + d;
+                    size_t idx = (((size_t)a * nj + b) * nk + c) * nl + d;
+                    double I = deg * w->val[idx], Ik = deg * (cK * w->val[idx] + (use_lr ? cLR * w->val2[idx] : 0.0));
+                    for (int m = 0; m < nmat; ++m) {
+                        const double *Bm = B[m];
+                        double *Fm = Ft + (size_t)m * n * n;
+                        double jb = wJ[m] * (Bm[l_ * n + s_] + Bm[s_ * n + l_]) * I, jk = wJ[m] * (Bm[m_ * n + n_] + Bm[n_ * n + m_]) * I;
+#define ADD(r, c, v) do { double v_ = (v); double *p_ = &Fm[(r) * n + (c)]; if (shared) { _Pragma("omp atomic") *p_ += v_; } else *p_ += v_; } while (0)
+#define XX(r, c) (wK[m] * Bm[(r) * n + (c)] + wKT[m] * Bm[(c) * n + (r)])
+                        ADD(m_, n_, jb); ADD(n_, m_, jb);
+                        ADD(l_, s_, jk); ADD(s_, l_, jk);
+                        ADD(m_, s_, -XX(l_, n_) * Ik); ADD(n_, s_, -XX(l_, m_) * Ik);
+                        ADD(m_, l_, -XX(s_, n_) * Ik); ADD(n_, l_, -XX(s_, m_) * Ik);
+                        ADD(l_, n_, -XX(m_, s_) * Ik); ADD(s_, n_, -XX(m_, l_) * Ik);
+                        ADD(l_, m_, -XX(n_, s_) * Ik); ADD(s_, m_, -XX(n_, l_) * Ik);
+#undef XX
+#undef ADD
+                    }
+                }
+            }
+        }
+        work_free(w);
+    }
+    for (int m = 0; m < nmat; ++m)
+        for (size_t t = 0; t < n * n; ++t) {
+            double sum = 0.0;
+            for (int th = 0; th < (shared ? 1 : nthr); ++th) sum += acc[nout * (size_t)th + (size_t)m * n * n + t];
+            F[m][t] = sum;
+        }
+    if (st) {
+        st->pairs_total = (int64_t)np_all; st->pairs_kept = (int64_t)npk;
+        st->quartets_visited = visited; st->quartets_computed = computed; st->prim_quartets = primq;
+    }
+    free(acc); free(pairs); free(Q); free(dm); sys_free(&s);
+    return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

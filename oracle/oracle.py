@@ -174,6 +174,38 @@ def density_weights(sysm, pairs, wJ, wK, cJ, cK, cLR, want_W=True):
     return d, W
 
 
+def _fock_args(Bs, wJ, wK, wKT, n):
+    B = [np.ascontiguousarray(b, dtype=np.float64) for b in Bs]
+    F = [np.zeros((n, n)) for _ in B]
+    PB = (C.c_void_p * len(B))(*[b.ctypes.data for b in B])
+    PF = (C.c_void_p * len(F))(*[f.ctypes.data for f in F])
+    w = [np.ascontiguousarray(x, dtype=np.float64) for x in (wJ, wK, wKT)]
+    return B, F, PB, PF, w
+
+
+def fock(sysm, Bs, wJ, wK, wKT, cK, cLR, omega, tau=None, density_weighted=None, sample_mod=0, sample_seed=0):
+    """Fock-type matrices F_k = wJ_k J[B_k] - (cK K + cLR K_lr)[wK_k B_k + wKT_k B_k^T] (eqs 19, 34), unique-quartet loop."""
+    args, keep = _sys_args(sysm)
+    B, F, PB, PF, w = _fock_args(Bs, wJ, wK, wKT, sysm.nbf)
+    opt = Options(sysm.tau if tau is None else tau, sysm.density_weighted if density_weighted is None else density_weighted,
+                  sample_mod, sample_seed)
+    st = Stats()
+    rc = lib().orc_fock(*args, C.byref(opt), C.c_int(len(B)), PB, *[x.ctypes.data_as(C.c_void_p) for x in w],
+                        C.c_double(cK), C.c_double(cLR), C.c_double(omega), PF, C.byref(st))
+    assert rc == 0, rc
+    return F, st.asdict()
+
+
+def fock_n4(sysm, Bs, wJ, wK, wKT, cK, cLR, omega):
+    """The same by the plain definition over all nshell^4 shell quartets (tiny inputs)."""
+    args, keep = _sys_args(sysm)
+    B, F, PB, PF, w = _fock_args(Bs, wJ, wK, wKT, sysm.nbf)
+    rc = lib().orc_fock_n4(*args, C.c_int(len(B)), PB, *[x.ctypes.data_as(C.c_void_p) for x in w],
+                           C.c_double(cK), C.c_double(cLR), C.c_double(omega), PF)
+    assert rc == 0, rc
+    return F
+
+
 def sample_keep(i, j, k, l, mod, seed) -> bool:
     return bool(lib().orc_sample_keep(C.c_int(i), C.c_int(j), C.c_int(k), C.c_int(l), C.c_uint32(mod), C.c_uint32(seed)))
 
