@@ -225,7 +225,9 @@ class CudaBackend:
     def context(self):
         return self.tdgrad.Context(self.local)
 
-    def densities(self, nbf, seed):
+    def densities(self, nbf, seed, sysm=None, kind="dense"):
+        if kind == "decaying":     # spatially decaying densities (workload.make_decaying_densities_torch)
+            return wl.make_decaying_densities_torch(sysm, seed, self.device)
         return wl.make_densities_torch(nbf, seed, self.device)
 
     def host_copies(self, mats):
@@ -276,7 +278,7 @@ def run_ours(args, backend=None, emit=print):
     peak_tf = ctx.fp64_peak(400.0)
     sysm = wl.make_system(cfg)
     nbf, natom = sysm.nbf, sysm.natom
-    D, P, T = be.densities(nbf, 20240716 + cfg)
+    D, P, T = be.densities(nbf, 20240716 + cfg, sysm, args.densities)
     pairs, wJ, wK = wl.default_call(D, P, T)
     g_dev = torch.zeros((natom, 3), dtype=torch.float64, device=dev)
 
@@ -354,6 +356,9 @@ def run_ours(args, backend=None, emit=print):
                      for c in range(tdgrad.NCLASS) if agg_q[c] and agg_ms[c] > 0}
         config = _config(cfg, sysm, ("shard%d+allreduce" % world) if shard else ("replicas" if world > 1 else "1gpu"))
         config["streams"] = args.streams
+        config["densities"] = args.densities
+        if args.densities != "dense":
+            config["workload"] += "; densities decaying as exp(-r / %.1f bohr) (workload.make_decaying_densities)" % wl.DECAY_LENGTH
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms / args.steps,
                     higher_is_better=True, scaling="strong" if shard else "weak", vs_baseline=None, dtype="f64", data="synthetic",
                     config=config, wall_time_s=ms / args.steps * 1e-3, quartets_per_step=total_quartets // args.steps,
@@ -373,6 +378,8 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--densities", default="dense", choices=["dense", "decaying"],
+                    help="dense: BASELINE.json's random matrices; decaying: second workload with spatially decaying densities (NEXT-4)")
     ap.add_argument("--streams", type=int, default=1, help="CUDA streams the class launches of a call are dealt over (tdg_set_streams)")
     ap.add_argument("--parallelism", default="shard", choices=["shard", "replicas"],
                     help="N > 1: work items sharded over the ranks + one NCCL all-reduce of the gradient (strong scaling, default), or independent replicas")

@@ -80,7 +80,20 @@ int tdg_destroy(tdg_ctx* ctx);
  * Invalidates any previous plan. */
 int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz_bohr, int nshell, const tdg_shell* shells,
                    int nprim_total, const double* exps, const double* coefs);
+/* Size of the square matrices the caller passes and receives: the number of Cartesian functions, or, after
+ * tdg_set_spherical, the number of functions of the mixed Cartesian / spherical input basis. */
 int tdg_nbf(const tdg_ctx* ctx, int* nbf);
+
+/* Spherical-harmonic shells (PAPER.md:241 n_sph = 2l+1, "transform Cartesian ERI derivatives
+ * into spherical basis", def2-SVP).  spherical[nshell] (HOST; NULL = all Cartesian): a nonzero flag on a d or f
+ * shell means its 2l+1 functions are the real solid harmonics m = -l..l, each normalised to unit self-overlap:
+ *   d: xy, yz, zz-(xx+yy)/2, xz, (sqrt3/2)(xx-yy);   f: y(3xx-yy), xyz, y(4zz-xx-yy), z(2zz-3xx-3yy), x(4zz-xx-yy), z(xx-yy), x(xx-3yy)
+ * (s and p shells are unaffected: a p shell is x, y, z either way).  The input matrices of tdg_gradient / tdg_energy /
+ * tdg_fock and the output of tdg_fock are then tdg_nbf x tdg_nbf in that basis.  Exact route, no kernel change: the transformation
+ * coefficients do not depend on the geometry, so the library back-transforms every input, D_cart = C^T D C, runs the Cartesian
+ * kernels, and forward-transforms Fock-type results, F = C F_cart C^T.  Schwarz bounds and the density-weighted test are those of
+ * the Cartesian representation.  Call after tdg_set_system (which resets all shells to Cartesian); the plan stays valid. */
+int tdg_set_spherical(tdg_ctx* ctx, const int32_t* spherical);
 
 /* Steps a1-a2: shell pairs, Schwarz bounds Q_ij = sqrt(max (mn|mn)) (full operator) computed
  * ON THE DEVICE, pair screening, sort into (la,lb,contraction degree) buckets by Q descending, work lists.
@@ -122,6 +135,21 @@ int tdg_gradient(tdg_ctx* ctx, int npair, const double* const* A, const double* 
 int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int matrices_on_device,
                const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
                void* stream, double* E_host);
+
+/* Fock-type (J/K) build, integral-direct with the same plan, screening and kernels' machinery as tdg_gradient (SURVEY.md 8(f)
+ * NEXT-1).  For each of the nmat input matrices B_k (nbf x nbf row-major, general; all device or all host pointers):
+ *
+ *   F_k[mn] = sum_ls [ wJ_k B_k[sl] (mn|ls)  -  X_k[sl] ( cK (ml|sn) + cLR (ml|sn)_lr ) ],    X_k = wK_k B_k + wKT_k B_k^T
+ *
+ * PAPER.md:197-207 (eqs 33-34, the sigma vector of the Z-vector iterations): wJ = 4, wK = wKT = 1, cK = alpha, cLR = beta.
+ * PAPER.md:138 (eq 19, F of a symmetric relaxed-difference density): wJ = 2, wK = 1, wKT = 0.  The XC-kernel term of both
+ * equations is not part of this library.  Screening: quartet kept iff Q_ij Q_kl >= tau and (density_weighted) Q_ij Q_kl W >= tau,
+ * W = max(max_k|wJ_k| max(d_ij,d_kl), (|cK|+|cLR|) max_k(|wK_k|+|wKT_k|) max(d_ik,d_il,d_jk,d_jl)), d = shell-block maxima of
+ * |B_k| over all k and both orientations.  F[k]: nbf x nbf row-major, device pointers if F_on_device != 0
+ * (completion stream-ordered) else host (the call synchronises); overwritten.  1 <= nmat <= 8.  stats may be NULL. */
+int tdg_fock(tdg_ctx* ctx, int nmat, const double* const* B, int matrices_on_device, const double* wJ, const double* wK,
+             const double* wKT, double cK, double cLR, double omega, void* stream, double* const* F, int F_on_device,
+             tdg_stats* stats);
 
 /* Rys roots/weights evaluator (step a5; reading S8), exposed for parity tests:
  * for each of `count` (T[i], rho[i]) HOST inputs writes n roots x_r and n weights w_r to out[i][2n] (host),

@@ -908,6 +908,47 @@ int orc_fock(SYS_ARGS, const orc_options *opt, int nmat, const double *const *B,
     return 0;
 }
 
+/* ---------------------------------------------------------------- NEXT-2: real solid harmonics
+ * C[2l+1][ncart(l)]: function m = -l..l of a spherical shell as a combination of the NORMALISED Cartesian components (order
+ * S7).  Built from the harmonic polynomials themselves (no stored coefficients): each monomial x^a y^b z^c carries the factor
+ * sqrt((2a-1)!!(2b-1)!!(2c-1)!!) that its normalised Cartesian function lacks, and the row is scaled to unit norm under the
+ * overlap of the normalised components, S = prod_dir (e+e'-1)!! / sqrt((2e-1)!!(2e'-1)!!) (even e+e' only).
+ * l <= 1: identity.  The tests pin the result by orthonormality under orc_overlap and by harmonicity of the polynomials. */
+typedef struct { int n; struct { int a, b, c; double co; } t[3]; } poly_t;
+static const poly_t SPH_D[5] = {
+    {1, {{1, 1, 0, 1}}}, {1, {{0, 1, 1, 1}}}, {3, {{0, 0, 2, 2}, {2, 0, 0, -1}, {0, 2, 0, -1}}}, {1, {{1, 0, 1, 1}}},
+    {2, {{2, 0, 0, 1}, {0, 2, 0, -1}}}};
+static const poly_t SPH_F[7] = {
+    {2, {{2, 1, 0, 3}, {0, 3, 0, -1}}}, {1, {{1, 1, 1, 1}}}, {3, {{0, 1, 2, 4}, {2, 1, 0, -1}, {0, 3, 0, -1}}},
+    {3, {{0, 0, 3, 2}, {2, 0, 1, -3}, {0, 2, 1, -3}}}, {3, {{1, 0, 2, 4}, {3, 0, 0, -1}, {1, 2, 0, -1}}},
+    {2, {{2, 0, 1, 1}, {0, 2, 1, -1}}}, {2, {{3, 0, 0, 1}, {1, 2, 0, -3}}}};
+int orc_sph_matrix(int l, double *C) {
+    int nc = ncart(l), ns = 2 * l + 1;
+    if (l < 0 || l > 3) return -1;
+    memset(C, 0, sizeof(double) * (size_t)(l < 2 ? nc * nc : ns * nc));
+    if (l < 2) { for (int i = 0; i < nc; ++i) C[i * nc + i] = 1.0; return 0; }
+    const poly_t *P = l == 2 ? SPH_D : SPH_F;
+    for (int m = 0; m < ns; ++m) {
+        double *row = C + (size_t)m * nc;
+        for (int t = 0; t < P[m].n; ++t)
+            for (int i = 0; i < nc; ++i) {
+                int x, y, z; cart_comp(l, i, &x, &y, &z);
+                if (x == P[m].t[t].a && y == P[m].t[t].b && z == P[m].t[t].c)
+                    row[i] += P[m].t[t].co * sqrt(dfact(2 * x - 1) * dfact(2 * y - 1) * dfact(2 * z - 1));
+            }
+        double nrm = 0.0;
+        for (int i = 0; i < nc; ++i) for (int j = 0; j < nc; ++j) {
+            int x, y, z, x2, y2, z2; cart_comp(l, i, &x, &y, &z); cart_comp(l, j, &x2, &y2, &z2);
+            if (((x + x2) | (y + y2) | (z + z2)) & 1) continue;
+            double sij = dfact(x + x2 - 1) * dfact(y + y2 - 1) * dfact(z + z2 - 1) /
+                         sqrt(dfact(2 * x - 1) * dfact(2 * y - 1) * dfact(2 * z - 1) * dfact(2 * x2 - 1) * dfact(2 * y2 - 1) * dfact(2 * z2 - 1));
+            nrm += row[i] * sij * row[j];
+        }
+        for (int i = 0; i < nc; ++i) row[i] /= sqrt(nrm);
+    }
+    return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

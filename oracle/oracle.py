@@ -206,6 +206,27 @@ def fock_n4(sysm, Bs, wJ, wK, wKT, cK, cLR, omega):
     return F
 
 
+def sph_matrix(l: int) -> np.ndarray:
+    """[2l+1 (l >= 2) or ncart(l), ncart(l)]: real solid harmonics m = -l..l over the normalised Cartesian components."""
+    nc = _ncart(l)
+    out = np.zeros((2 * l + 1 if l >= 2 else nc, nc))
+    rc = lib().orc_sph_matrix(C.c_int(l), out.ctypes.data_as(C.c_void_p))
+    assert rc == 0, rc
+    return out
+
+
+def sph_transform(sysm, flags) -> np.ndarray:
+    """Block-diagonal C [nbf_in, nbf_cart] of the mixed input basis: flagged d/f shells spherical, the rest Cartesian."""
+    blocks = [sph_matrix(int(l)) if (f and l >= 2) else np.eye(_ncart(int(l))) for l, f in zip(sysm.shells[:, 1], flags)]
+    nin, nc = sum(b.shape[0] for b in blocks), sum(b.shape[1] for b in blocks)
+    Cm = np.zeros((nin, nc))
+    r = c = 0
+    for b in blocks:
+        Cm[r:r + b.shape[0], c:c + b.shape[1]] = b
+        r += b.shape[0]; c += b.shape[1]
+    return Cm
+
+
 def sample_keep(i, j, k, l, mod, seed) -> bool:
     return bool(lib().orc_sample_keep(C.c_int(i), C.c_int(j), C.c_int(k), C.c_int(l), C.c_uint32(mod), C.c_uint32(seed)))
 

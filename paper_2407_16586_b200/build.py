@@ -17,10 +17,24 @@ LMAX = 3
 PAIR_CLASSES = [(la, lb) for la in range(LMAX + 1) for lb in range(la + 1)]
 QUARTET_CLASSES = [p + q for i, p in enumerate(PAIR_CLASSES) for q in PAIR_CLASSES[: i + 1]]   # bra class >= ket class
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
-         "-DTDG_LMAX_BUILD=%d" % LMAX]
-# per-class compile flags (launch bounds measured on cfg 3, see profiles/): class -> extra nvcc flags
-CLASS_FLAGS: dict = {}
+FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
+# per-class compile flags: minimum resident blocks per SM of __launch_bounds__ (registers traded for occupancy), measured on
+# cfg 3 (profiles/r02_variants.md): class -> extra nvcc flags
+CLASS_FLAGS: dict = {(0, 0, 0, 0): ["-DTDG_MINB=4"], (1, 0, 0, 0): ["-DTDG_MINB=3"], (2, 0, 0, 0): ["-DTDG_MINB=3"]}
+
+
+def ncart(l: int) -> int:
+    return (l + 1) * (l + 2) // 2
+
+
+def num_roles(la: int, lb: int, lc: int, ld: int) -> int:
+    """QC<la,lb,lc,ld>::NROLE of csrc/tdg_grad.cuh (a static_assert in tdg_class.cu and the launcher table catch a mismatch)."""
+    rc = 54 if (la, lb, lc, ld) == (2, 2, 2, 1) else 27
+    nab, kdn = ncart(la) * ncart(lb), ncart(lc) * ncart(ld)
+    abn1 = nab if rc // kdn >= nab else max(rc // kdn, 1)
+    nrole1 = -(-nab // abn1)
+    small = nab * kdn <= 27 or (3 not in (la, lb, lc, ld) and nrole1 <= 18)
+    return nrole1 if small else 1
 DEPS = {   # headers each source includes
     "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "rys_meta.inc"],
     "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
@@ -54,8 +68,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     jobs = [("tdg_api.cu", os.path.join(OBJ, "tdg_api.o"), []), ("tdg_aux.cu", os.path.join(OBJ, "tdg_aux.o"), [])]
     for la, lb, lc, ld in QUARTET_CLASSES:
-        jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d%d%d.o" % (la, lb, lc, ld)),
-                     ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb, "-DTDG_LC=%d" % lc, "-DTDG_LD=%d" % ld] + CLASS_FLAGS.get((la, lb, lc, ld), [])))
+        for role in range(num_roles(la, lb, lc, ld)):   # one translation unit per (class, role): they compile in parallel
+            jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d%d%d_r%d.o" % (la, lb, lc, ld, role)),
+                         ["-DTDG_LA=%d" % la, "-DTDG_LB=%d" % lb, "-DTDG_LC=%d" % lc, "-DTDG_LD=%d" % ld, "-DTDG_ROLE=%d" % role]
+                         + CLASS_FLAGS.get((la, lb, lc, ld), [])))
     # longest compiles first (fully unrolled d-shell classes)
     jobs.sort(key=lambda j: 0 if "class" not in j[1] else -sum(int(c) for c in os.path.basename(j[1])[10:14]))
     todo = []

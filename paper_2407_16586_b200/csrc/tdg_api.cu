@@ -15,16 +15,25 @@
 #define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
 #define TDG_MAX_STREAMS 8
 
-#define TDG_CLASS(la, lb, lc, ld) tdg_launch_fn tdg_class_launcher_##la##lb##lc##ld();
-#include "tdg_classes.inc"
-#undef TDG_CLASS
-
-tdg_launch_fn tdg_get_launcher(int la, int lb, int lc, int ld) {
+// Launchers register themselves at load time (one translation unit per class and role, tdg_class.cu).
+#define TDG_ROLE_SLOTS 64
+static tdg_launch_fn g_launchers[TDG_NCLASS][TDG_ROLE_SLOTS];
+static int class_index(int la, int lb, int lc, int ld) {
+  const int c1 = PCLS(la, lb), c2 = PCLS(lc, ld);
+  return c1 * (c1 + 1) / 2 + c2;
+}
+void tdg_register_launcher(int la, int lb, int lc, int ld, int role, tdg_launch_fn fn) {
+  if (la <= TDG_MAX_L && role >= 0 && role < TDG_ROLE_SLOTS) g_launchers[class_index(la, lb, lc, ld)][role] = fn;
+}
+tdg_launch_fn tdg_get_launcher(int la, int lb, int lc, int ld, int role) {
+  return (role >= 0 && role < TDG_ROLE_SLOTS) ? g_launchers[class_index(la, lb, lc, ld)][role] : nullptr;
+}
+int tdg_num_roles(int la, int lb, int lc, int ld) {
 #define TDG_CLASS(a, b, c, d) \
-  if (la == a && lb == b && lc == c && ld == d) return (a <= TDG_LMAX_BUILD) ? tdg_class_launcher_##a##b##c##d() : nullptr;
+  if (la == a && lb == b && lc == c && ld == d) return QC<a, b, c, d>::NROLE;
 #include "tdg_classes.inc"
 #undef TDG_CLASS
-  return nullptr;
+  return 0;
 }
 
 namespace {
@@ -53,6 +62,10 @@ struct tdg_ctx {
   DevShell* d_shells = nullptr;
   int* d_bf2sh = nullptr;
   bool have_Q = false;
+  // input basis (tdg_set_spherical): matrices are passed in a basis where flagged d/f shells are real solid harmonics
+  bool any_sph = false;
+  int nbf_in = 0;
+  int *d_inoff = nullptr, *d_sph = nullptr, *d_in2sh = nullptr;
   // plan
   bool planned = false;
   tdg_options opt{};
@@ -92,6 +105,8 @@ static void free_system(tdg_ctx* c) {
   free_plan(c);
   cudaFree(c->d_xyz); cudaFree(c->d_exps); cudaFree(c->d_cn); cudaFree(c->d_Q); cudaFree(c->d_shells);
   cudaFree(c->d_grad); cudaFree(c->d_dmax); cudaFree(c->d_bf2sh); c->d_bf2sh = nullptr;
+  cudaFree(c->d_inoff); cudaFree(c->d_sph); cudaFree(c->d_in2sh); c->d_inoff = c->d_sph = c->d_in2sh = nullptr;
+  c->any_sph = false; c->nbf_in = 0;
   c->d_xyz = c->d_exps = c->d_cn = c->d_Q = c->d_grad = c->d_dmax = nullptr; c->d_shells = nullptr;
   for (auto& s : c->scratch) cudaFree(s.second);
   c->scratch.clear(); c->scratch_used.clear();
@@ -160,7 +175,7 @@ extern "C" int tdg_set_streams(tdg_ctx* ctx, int nstreams) {
 
 extern "C" int tdg_nbf(const tdg_ctx* ctx, int* nbf) {
   if (!ctx || !nbf) return TDG_EINVAL;
-  *nbf = ctx->nbf;
+  *nbf = ctx->nbf_in;   // size of the matrices the caller passes (= the Cartesian count unless tdg_set_spherical flagged shells)
   return TDG_OK;
 }
 
@@ -174,7 +189,7 @@ extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int ns
   for (int s = 0; s < nshell; ++s) {
     const tdg_shell& sh = shells[s];
     if (sh.atom < 0 || sh.atom >= natom || sh.nprim <= 0 || sh.prim_off < 0 || sh.prim_off + sh.nprim > nprim_total || sh.l < 0) return TDG_EINVAL;
-    if (sh.l > TDG_MAX_L || sh.l > TDG_LMAX_BUILD) return TDG_EUNSUPPORTED;
+    if (sh.l > TDG_MAX_L) return TDG_EUNSUPPORTED;
     for (int k = 0; k < sh.nprim; ++k) if (!(exps[sh.prim_off + k] > 0.0)) return TDG_EINVAL;
   }
   // a0: all host arithmetic and validation first; the context is only touched once nothing can fail on the host side
@@ -222,7 +237,36 @@ extern "C" int tdg_set_system(tdg_ctx* ctx, int natom, const double* xyz, int ns
   CK(cudaMemcpy(ctx->d_cn, ctx->cn.data(), sizeof(double) * nprim_total, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(ctx->d_shells, ctx->shells.data(), sizeof(DevShell) * nshell, cudaMemcpyHostToDevice));
   // only now does the context count as holding a system (tdg_plan / tdg_schwarz check nshell > 0)
-  ctx->natom = natom; ctx->nshell = nshell; ctx->nprim = nprim_total; ctx->nbf = off;
+  ctx->natom = natom; ctx->nshell = nshell; ctx->nprim = nprim_total; ctx->nbf = off; ctx->nbf_in = off;
+  return TDG_OK;
+}
+
+// NEXT-2: flagged d and f shells enter and leave the library as real solid harmonics.
+extern "C" int tdg_set_spherical(tdg_ctx* ctx, const int32_t* spherical) {
+  if (!ctx) return TDG_EINVAL;
+  if (ctx->nshell <= 0) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  const int ns = ctx->nshell;
+  std::vector<int> flag(ns, 0), inoff(ns, 0), in2sh;
+  bool any = false;
+  int off = 0;
+  for (int s = 0; s < ns; ++s) {
+    const int l = ctx->shells[s].l;
+    flag[s] = (spherical && spherical[s] && l >= 2) ? 1 : 0;
+    any = any || flag[s];
+    inoff[s] = off;
+    const int nf = flag[s] ? 2 * l + 1 : ncart(l);
+    for (int f = 0; f < nf; ++f) in2sh.push_back(s);
+    off += nf;
+  }
+  cudaFree(ctx->d_inoff); cudaFree(ctx->d_sph); cudaFree(ctx->d_in2sh); ctx->d_inoff = ctx->d_sph = ctx->d_in2sh = nullptr;
+  ctx->any_sph = false; ctx->nbf_in = ctx->nbf;
+  if (!any) return TDG_OK;
+  CK(cudaMalloc(&ctx->d_inoff, sizeof(int) * ns)); CK(cudaMalloc(&ctx->d_sph, sizeof(int) * ns)); CK(cudaMalloc(&ctx->d_in2sh, sizeof(int) * off));
+  CK(cudaMemcpy(ctx->d_inoff, inoff.data(), sizeof(int) * ns, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(ctx->d_sph, flag.data(), sizeof(int) * ns, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(ctx->d_in2sh, in2sh.data(), sizeof(int) * off, cudaMemcpyHostToDevice));
+  ctx->any_sph = true; ctx->nbf_in = off;
   return TDG_OK;
 }
 
@@ -375,6 +419,27 @@ struct DevTemp {     // cudaMalloc'ed temporary freed on every exit path
 };
 }
 
+// Input matrix (host or device, input basis) -> device pointer to its CARTESIAN nbf x nbf form: upload if needed, then
+// D_cart = C^T D C when spherical shells are flagged (NEXT-2).
+static int to_device_cart(tdg_ctx* ctx, const double* M, int on_dev, cudaStream_t st, const double** out) {
+  const size_t nin = (size_t)ctx->nbf_in, n = (size_t)ctx->nbf;
+  const double* src = M;
+  if (!on_dev) {
+    double* buf = (double*)scratch_get(ctx, sizeof(double) * nin * nin);
+    if (!buf) { ctx->err = "device allocation of an input matrix failed"; return TDG_ENOMEM; }
+    CK(cudaMemcpyAsync(buf, M, sizeof(double) * nin * nin, cudaMemcpyHostToDevice, st));
+    src = buf;
+  }
+  if (ctx->any_sph) {
+    double* cart = (double*)scratch_get(ctx, sizeof(double) * n * n);
+    if (!cart) { ctx->err = "device allocation of a back-transformed matrix failed"; return TDG_ENOMEM; }
+    CK(tdg_launch_sph_transform(src, cart, (int)n, (int)nin, 0, ctx->d_bf2sh, ctx->d_shells, ctx->d_inoff, ctx->d_sph, st));
+    src = cart;
+  }
+  *out = src;
+  return TDG_OK;
+}
+
 static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, const double* const* B, int on_dev,
                            const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
                            cudaStream_t st, tdg_stats* stats, double* E_host = nullptr) {
@@ -390,13 +455,9 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
   for (int k = 0; k < npair; ++k)
     for (const double* M : {A[k], B[k]}) {
       if (uid(M) >= 0) continue;
-      const double* d = M;
-      if (!on_dev) {
-        double* buf = (double*)scratch_get(ctx, mbytes);
-        if (!buf) { ctx->err = "device allocation of a density matrix failed"; return TDG_ENOMEM; }
-        CK(cudaMemcpyAsync(buf, M, mbytes, cudaMemcpyHostToDevice, st));
-        d = buf;
-      }
+      const double* d = nullptr;
+      const int rc_in = to_device_cart(ctx, M, on_dev, st, &d);
+      if (rc_in) return rc_in;
       uniq.push_back(M); udev.push_back(d);
     }
   if (uniq.size() > 16) return TDG_EINVAL;
@@ -492,8 +553,7 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
     for (size_t w = 0; w < nw; ++w) {
       const Work& W = ctx->work[w];
       const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
-      tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb);
-      if (!fn && !d_E) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+      const int nrole = d_E ? 1 : tdg_num_roles(X.la, X.lb, Y.la, Y.lb);
       P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
       P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
       P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
@@ -503,9 +563,15 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
       cudaEvent_t e0 = nullptr, e1 = nullptr;
       if (stats) { e0 = pool.get(); e1 = pool.get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, ls); }
       if (d_E) CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, ls));
-      else fn(P, W.nblocks, ls);
+      else
+        for (int role = 0; role < nrole; ++role) {   // the roles of a class are separate kernels (slices of the bra function pairs)
+          tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb, role);
+          if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+          fn(P, W.nblocks, ls);
+          ++launches;
+        }
+      if (d_E) ++launches;
       if (stats) { cudaEventRecord(e1, ls); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(W.cls); }
-      ++launches;
     }
     if (nstr > 1)
       for (int i = 0; i < nstr - 1; ++i) { CK(cudaEventRecord(ctx->ev_join[i], ctx->side[i])); CK(cudaStreamWaitEvent(st, ctx->ev_join[i], 0)); }
@@ -569,6 +635,162 @@ extern "C" int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const
   if (!ctx->planned) return TDG_ENOTPLANNED;
   cudaSetDevice(ctx->device);
   return run_contraction(ctx, npair, A, B, matrices_on_device, wJ, wK, cJ, cK, cLR, omega, (cudaStream_t)stream, nullptr, E_host);
+}
+
+// ---- NEXT-1: Fock-type (J/K) build (eq 19, eqs 33-34; kernels in tdg_fock.cuh) ----
+extern "C" int tdg_fock(tdg_ctx* ctx, int nmat, const double* const* B, int matrices_on_device, const double* wJ, const double* wK,
+                        const double* wKT, double cK, double cLR, double omega, void* stream, double* const* F, int F_on_device,
+                        tdg_stats* stats) {
+  if (!ctx) return TDG_EINVAL;
+  if (!B || !F || !wJ || !wK || !wKT || nmat <= 0 || nmat > TDG_MAXP) return TDG_EINVAL;
+  for (int k = 0; k < nmat; ++k) if (!B[k] || !F[k]) return TDG_EINVAL;
+  if (cLR != 0.0 && !(omega > 0.0)) return TDG_EINVAL;
+  if (!ctx->planned) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n = ctx->nbf;
+  const size_t mbytes = sizeof(double) * (size_t)n * n;
+  std::fill(ctx->scratch_used.begin(), ctx->scratch_used.end(), false);
+  EventPool pool;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
+  if (stats) { ev0 = pool.get(); ev1 = pool.get(); ev2 = pool.get(); if (!ev0 || !ev1 || !ev2) return TDG_ECUDA; cudaEventRecord(ev0, st); }
+  std::vector<const double*> bdev(nmat);
+  std::vector<double*> fdev(nmat);
+  for (int k = 0; k < nmat; ++k) {
+    const int rc_in = to_device_cart(ctx, B[k], matrices_on_device, st, &bdev[k]);
+    if (rc_in) return rc_in;
+    fdev[k] = F[k];
+    if (!F_on_device || ctx->any_sph) {   // Cartesian result buffer (transformed / copied out at the end)
+      fdev[k] = (double*)scratch_get(ctx, mbytes);
+      if (!fdev[k]) { ctx->err = "device allocation of an output matrix failed"; return TDG_ENOMEM; }
+    }
+    CK(cudaMemsetAsync(fdev[k], 0, mbytes, st));
+  }
+  const bool useK = (cK != 0.0 || cLR != 0.0);
+  // which inputs are nonsymmetric (only matters where wK != wKT: the exchange density wK B + wKT B^T is then nonsymmetric)
+  double as[TDG_MAXP] = {0};
+  bool need_as = false;
+  for (int k = 0; k < nmat; ++k) need_as = need_as || (useK && wK[k] != wKT[k]);
+  if (need_as) {
+    double* d_as = (double*)scratch_get(ctx, 256);
+    if (!d_as) return TDG_ENOMEM;
+    CK(cudaMemsetAsync(d_as, 0, 256, st));
+    for (int k = 0; k < nmat; ++k) CK(tdg_launch_asym(bdev[k], n, d_as + k, st));
+    CK(cudaMemcpyAsync(as, d_as, sizeof(double) * nmat, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+  }
+  // canonical slots: S_k = (B_k + B_k^T)/2 carries J (weight 2 wJ) and the symmetric part of the exchange density (wK + wKT);
+  // N_k = (B_k - B_k^T)/2 carries the antisymmetric part (wK - wKT) and is finished with F -= G^T
+  struct Slot { int mat, kind; double jw, kw; };
+  std::vector<Slot> slots;
+  double CJ = 0.0, CKs = 0.0;
+  for (int k = 0; k < nmat; ++k) {
+    CJ = std::max(CJ, std::fabs(wJ[k])); CKs = std::max(CKs, std::fabs(wK[k]) + std::fabs(wKT[k]));
+    const double ks = useK ? wK[k] + wKT[k] : 0.0, kn = useK ? wK[k] - wKT[k] : 0.0;
+    if (wJ[k] != 0.0 || ks != 0.0) slots.push_back(Slot{k, 0, 2.0 * wJ[k], ks});
+    if (kn != 0.0 && as[k] != 0.0) slots.push_back(Slot{k, 1, 0.0, kn});
+  }
+  CKs *= std::fabs(cK) + std::fabs(cLR);
+  KParams P{};
+  P.CJ = CJ; P.CK = CKs; P.wmode = 1;
+  P.tau = ctx->opt.tau; P.density_weighted = (ctx->opt.tau > 0.0) ? ctx->opt.density_weighted : 0;
+  P.nshell = ctx->nshell; P.sample_mod = ctx->opt.sample_mod; P.sample_seed = ctx->opt.sample_seed;
+  P.nbf = n; P.cK = cK; P.cLR = cLR; P.omega = omega; P.omega2 = omega * omega; P.use_lr = (cLR != 0.0) ? 1 : 0;
+  P.rys_tab = ctx->d_rys;
+  int aux_launches = 0;
+  if (P.density_weighted) {
+    if (!ctx->d_dmax) CK(cudaMalloc(&ctx->d_dmax, sizeof(double) * (size_t)ctx->nshell * ctx->nshell));
+    MatList ml{};
+    ml.n = nmat;
+    for (int i = 0; i < nmat; ++i) ml.m[i] = bdev[i];
+    CK(tdg_launch_dmax(ml, n, ctx->d_shells, ctx->nshell, ctx->d_dmax, st));
+    P.dmax = ctx->d_dmax;
+    aux_launches += 2;
+  }
+  double* pk = (double*)scratch_get(ctx, 4 * mbytes);
+  double* G = (double*)scratch_get(ctx, 4 * mbytes + 8);   // (+8: a size distinct from pk's, the scratch cache keys on bytes)
+  if (!pk || !G) { ctx->err = "device allocation of the packed / accumulator arrays failed"; return TDG_ENOMEM; }
+  P.pk = pk; P.grad = G;
+  const size_t nw = ctx->work.size();
+  CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * (nw * 3 + 3), st));
+  if (stats) cudaEventRecord(ev1, st);
+  int launches = 0;
+  std::vector<cudaEvent_t> evs;
+  std::vector<int> ev_cls;
+  const int npass = (int)((slots.size() + 3) / 4);
+  for (int pass = 0; pass < npass; ++pass) {
+    PackSrc ps{};
+    for (int t = 0; t < 4; ++t) { P.MJ[t] = 0.0; P.MK[t] = 0.0; }
+    const int s0 = pass * 4, s1 = std::min((int)slots.size(), s0 + 4);
+    for (int s = s0; s < s1; ++s) {
+      ps.src[s - s0] = bdev[slots[s].mat]; ps.kind[s - s0] = slots[s].kind;
+      P.MJ[s - s0] = slots[s].jw; P.MK[s - s0] = slots[s].kw;
+    }
+    CK(tdg_launch_pack(ps, n, ctx->d_bf2sh, ctx->d_shells, pk, st));
+    CK(cudaMemsetAsync(G, 0, 4 * mbytes, st));
+    aux_launches += 2;
+    for (size_t w = 0; w < nw; ++w) {
+      const Work& W = ctx->work[w];
+      const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
+      P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
+      P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
+      P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
+      P.counters = ctx->d_counters + 3 * (pass == 0 ? w : nw);
+      cudaEvent_t e0 = nullptr, e1 = nullptr;
+      if (stats) { e0 = pool.get(); e1 = pool.get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, st); }
+      const int nrole = tdg_num_roles(X.la, X.lb, Y.la, Y.lb);
+      for (int role = 0; role < nrole; ++role) {
+        tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb, role + TDG_FOCK_ROLE_BASE);
+        if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+        fn(P, W.nblocks, st);
+        ++launches;
+      }
+      if (stats) { cudaEventRecord(e1, st); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(W.cls); }
+    }
+    for (int s = s0; s < s1; ++s) {
+      CK(tdg_launch_fock_finalize(G + (size_t)(s - s0) * n * n, n, slots[s].kind == 0 ? 1.0 : -1.0, fdev[slots[s].mat], st));
+      ++aux_launches;
+    }
+  }
+  CK(cudaGetLastError());
+  {
+    const size_t nin = (size_t)ctx->nbf_in, obytes = sizeof(double) * nin * nin;
+    for (int k = 0; k < nmat; ++k) {
+      const double* res = fdev[k];
+      if (ctx->any_sph) {   // F_sph = C F_cart C^T
+        double* o = F_on_device ? F[k] : (double*)scratch_get(ctx, obytes);
+        if (!o) { ctx->err = "device allocation of an output matrix failed"; return TDG_ENOMEM; }
+        CK(tdg_launch_sph_transform(fdev[k], o, (int)nin, n, 1, ctx->d_in2sh, ctx->d_shells, ctx->d_inoff, ctx->d_sph, st));
+        res = o;
+      }
+      if (!F_on_device) CK(cudaMemcpyAsync(F[k], res, obytes, cudaMemcpyDeviceToHost, st));
+    }
+    if (!F_on_device) CK(cudaStreamSynchronize(st));
+  }
+  if (stats) {
+    cudaEventRecord(ev2, st);
+    CK(cudaStreamSynchronize(st));
+    std::vector<unsigned long long> cnt(nw * 3 + 3);
+    CK(cudaMemcpy(cnt.data(), ctx->d_counters, sizeof(unsigned long long) * cnt.size(), cudaMemcpyDeviceToHost));
+    std::memset(stats, 0, sizeof(*stats));
+    stats->pairs_total = ctx->pairs_total; stats->pairs_kept = ctx->pairs_kept;
+    for (size_t w = 0; w < nw; ++w) {
+      stats->quartets_visited += (int64_t)cnt[3 * w]; stats->quartets_computed += (int64_t)cnt[3 * w + 1];
+      stats->prim_quartets += (int64_t)cnt[3 * w + 2];
+      stats->quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 1];
+      stats->prim_quartets_by_class[ctx->work[w].cls] += (int64_t)cnt[3 * w + 2];
+    }
+    for (size_t e = 0; e < ev_cls.size(); ++e) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, evs[2 * e], evs[2 * e + 1]);
+      stats->ms_by_class[ev_cls[e]] += ms;
+    }
+    cudaEventElapsedTime(&stats->ms_prepare, ev0, ev1);
+    cudaEventElapsedTime(&stats->ms_total, ev0, ev2);
+    stats->launches = launches + aux_launches;
+    stats->groups = npass;
+  }
+  return TDG_OK;
 }
 
 extern "C" int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out) {

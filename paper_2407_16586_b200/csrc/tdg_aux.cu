@@ -323,6 +323,96 @@ cudaError_t tdg_launch_pack(const PackSrc& ps, int n, const int* bf2sh, const De
   return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Spherical-harmonic shells (PAPER.md:241 n_sph, Fig. 1, def2-SVP).
+// Real solid harmonics of a d or f shell, m = -l..l, as combinations of the NORMALISED Cartesian components of the shell
+// (order S7); s and p shells are their Cartesian selves.  The integrals stay Cartesian: because the coefficients do not
+// depend on the geometry, contracting spherical-basis matrices with derivative integrals is exactly the Cartesian
+// contraction of the back-transformed matrices D_cart = C^T D_sph C, and a Fock-type matrix goes forward, F_sph = C F_cart C^T.
+//   d: xy, yz, zz - (xx+yy)/2, xz, (sqrt3/2)(xx - yy)
+//   f: (3/(2 sqrt2)) xxy - sqrt(5/8) yyy;  xyz;  sqrt(6/5) yzz - (sqrt6/4) yyy - (sqrt(6/5)/4) xxy;  zzz - (3/(2 sqrt5))(xxz + yyz);
+//      sqrt(6/5) xzz - (sqrt6/4) xxx - (sqrt(6/5)/4) xyy;  (sqrt3/2)(xxz - yyz);  sqrt(5/8) xxx - (3/(2 sqrt2)) xyy
+#define S3H 0.86602540378443864676   /* sqrt(3)/2 */
+#define F_A 1.06066017177982128660   /* 3/(2 sqrt 2) */
+#define F_B 0.79056941504209483300   /* sqrt(5/8) */
+#define F_C 1.09544511501033222691   /* sqrt(6/5) */
+#define F_D 0.61237243569579452455   /* sqrt(6)/4 */
+#define F_E 0.27386127875258305673   /* sqrt(6/5)/4 */
+#define F_F 0.67082039324993690892   /* 3/(2 sqrt 5) */
+__constant__ static double c_sph[2][7][10] = {
+  // l = 2; Cartesian order xx, xy, xz, yy, yz, zz
+  {{0, 1, 0, 0, 0, 0}, {0, 0, 0, 0, 1, 0}, {-0.5, 0, 0, -0.5, 0, 1}, {0, 0, 1, 0, 0, 0}, {S3H, 0, 0, -S3H, 0, 0}},
+  // l = 3; Cartesian order xxx, xxy, xxz, xyy, xyz, xzz, yyy, yyz, yzz, zzz
+  {{0, F_A, 0, 0, 0, 0, -F_B, 0, 0, 0}, {0, 0, 0, 0, 1, 0, 0, 0, 0, 0}, {0, -F_E, 0, 0, 0, 0, -F_D, 0, F_C, 0},
+   {0, 0, -F_F, 0, 0, 0, 0, -F_F, 0, 1}, {-F_D, 0, 0, -F_E, 0, F_C, 0, 0, 0, 0}, {0, 0, S3H, 0, 0, 0, 0, -S3H, 0, 0},
+   {F_B, 0, 0, -F_A, 0, 0, 0, 0, 0, 0}}};
+
+__device__ __forceinline__ double sph_coef(int l, int sph, int p, int a) {   // C[p][a]: function p of the input basis, Cartesian component a
+  return (sph && l >= 2) ? c_sph[l - 2][p][a] : (p == a ? 1.0 : 0.0);
+}
+__device__ __forceinline__ int shell_nin(int l, int sph) { return (sph && l >= 2) ? 2 * l + 1 : ncart(l); }
+
+// dir 0: Cartesian out[nc x nc] = C^T in C (in: input basis nin x nin).  dir 1: input-basis out[nin x nin] = C in C^T (in: Cartesian).
+__global__ void sph_transform_kernel(const double* __restrict__ in, double* __restrict__ out, int nout, int nin_dim, int dir,
+                                     const int* __restrict__ out2sh, const DevShell* __restrict__ sh, const int* __restrict__ inoff,
+                                     const int* __restrict__ sphflag) {
+  const int col = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;
+  if (col >= nout) return;
+  const int I = out2sh[row], J = out2sh[col];
+  const DevShell sI = sh[I], sJ = sh[J];
+  const int fI = sphflag[I], fJ = sphflag[J];
+  double acc = 0.0;
+  if (dir == 0) {   // row, col are Cartesian function indices
+    const int a = row - sI.bf_off, b = col - sJ.bf_off;
+    const int nI = shell_nin(sI.l, fI), nJ = shell_nin(sJ.l, fJ);
+    for (int p = 0; p < nI; ++p) {
+      const double cp = sph_coef(sI.l, fI, p, a);
+      if (cp == 0.0) continue;
+      for (int q = 0; q < nJ; ++q) {
+        const double cq = sph_coef(sJ.l, fJ, q, b);
+        if (cq != 0.0) acc += cp * cq * in[(size_t)(inoff[I] + p) * nin_dim + inoff[J] + q];
+      }
+    }
+  } else {          // row, col are input-basis function indices
+    const int p = row - inoff[I], q = col - inoff[J];
+    for (int a = 0; a < ncart(sI.l); ++a) {
+      const double cp = sph_coef(sI.l, fI, p, a);
+      if (cp == 0.0) continue;
+      for (int b = 0; b < ncart(sJ.l); ++b) {
+        const double cq = sph_coef(sJ.l, fJ, q, b);
+        if (cq != 0.0) acc += cp * cq * in[(size_t)(sI.bf_off + a) * nin_dim + sJ.bf_off + b];
+      }
+    }
+  }
+  out[(size_t)row * nout + col] = acc;
+}
+cudaError_t tdg_launch_sph_transform(const double* in, double* out, int nout, int nin_dim, int dir, const int* out2sh, const DevShell* sh,
+                                     const int* inoff, const int* sphflag, cudaStream_t s) {
+  dim3 block(128), grid((nout + 127) / 128, nout);
+  sph_transform_kernel<<<grid, block, 0, s>>>(in, out, nout, nin_dim, dir, out2sh, sh, inoff, sphflag);
+  return cudaGetLastError();
+}
+
+// Fock-type build, last step: F += G + sign * G^T  (the four index permutations the class kernels leave to the transpose)
+__global__ void fock_finalize_kernel(const double* __restrict__ G, int n, double sign, double* __restrict__ F) {
+  __shared__ double tile[32][33];
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int row = bx + r, col = by + threadIdx.x;
+    tile[r][threadIdx.x] = (row < n && col < n) ? G[(size_t)row * n + col] : 0.0;   // G[bx+r][by+c]
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const int row = by + r, col = bx + threadIdx.x;
+    if (row < n && col < n) F[(size_t)row * n + col] += G[(size_t)row * n + col] + sign * tile[threadIdx.x][r];
+  }
+}
+cudaError_t tdg_launch_fock_finalize(const double* G, int n, double sign, double* F, cudaStream_t s) {
+  dim3 block(32, 8), grid((n + 31) / 32, (n + 31) / 32);
+  fock_finalize_kernel<<<grid, block, 0, s>>>(G, n, sign, F);
+  return cudaGetLastError();
+}
+
 __global__ void dmax_block_kernel(const MatList mats, int n, const DevShell* __restrict__ sh, int ns, double* __restrict__ m) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
   if (j >= ns) return;

@@ -28,7 +28,7 @@ struct KParams {
   const PairHdr* ket_hdr; const double* ket_prim; int nket; int nppk;
   const int* cum;        // [ntiles+1] cumulative number of block work items per bra tile
   int ntiles; int same_bucket;
-  double tau; int density_weighted; const double* dmax; int nshell;
+  double tau; int density_weighted; int wmode; const double* dmax; int nshell;   // wmode 0: gradient weight (S9), 1: Fock-build weight
   double CJ, CK;         // S9 weights of the density-weighted bound
   uint32_t sample_mod, sample_seed;
   // Packed densities (tdg_internal.h): 4 canonical matrices interleaved, shell-blocked.  With u = pk(ik)[a,c][.],
@@ -159,10 +159,14 @@ __device__ __forceinline__ void rys_roots_boys(const double* __restrict__ tabN, 
     x[0] = F / F0; w[0] = F0;
   } else {
     const double m3 = F, m2 = fma(T2, m3, e) * 0.2, m1 = fma(T2, m2, e) * (1.0 / 3.0), m0 = fma(T2, m1, e);
+    // roots of x^2 + c1 x + c0 (the monic orthogonal quadratic): with D = c1^2 - 4 c0 and r = D^(-1/2): x2 - x1 = D r = 1/r, so
+    // one division (the Hankel determinant) and one rsqrt replace three divisions and a square root; x1 = -(c1 + sqrt D)/2
+    // loses at most one digit (x2/x1 <= ~10 for every T), well inside the 3e-13 moment tolerance of the tests
     const double rdet = 1.0 / (m0 * m2 - m1 * m1);
     const double c1 = (m1 * m2 - m0 * m3) * rdet, c0 = (m1 * m3 - m2 * m2) * rdet;
-    const double x2 = 0.5 * (sqrt(c1 * c1 - 4.0 * c0) - c1), x1 = c0 / x2;
-    const double w1 = (m0 * x2 - m1) / (x2 - x1);
+    const double disc = fma(c1, c1, -4.0 * c0), r = rsqrt(disc), sq = disc * r;
+    const double x2 = 0.5 * (sq - c1), x1 = -0.5 * (sq + c1);
+    const double w1 = fma(m0, x2, -m1) * r;
     x[0] = x1; x[N - 1] = x2; w[0] = w1; w[N - 1] = m0 - w1;
   }
 }

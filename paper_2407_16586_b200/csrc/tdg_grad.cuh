@@ -19,12 +19,10 @@
 #ifndef TDG_RU_LIM
 #define TDG_RU_LIM 120
 #endif
-#ifndef TDG_ROLE_COMPS
-#define TDG_ROLE_COMPS 27   // target number of function quartets per role
-#endif
-#ifndef TDG_MAX_ROLES
-#define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dp), (dd|dd), f shells) keep rolled loops (compile time)
-#endif
+#define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dd), f shells) use the block-per-quartet kernel (tdg_gradb.cuh)
+// target number of function quartets per role: 27 is the measured optimum (14: +30 %, 54: +15 % time on cfg 3), except
+// (dd|dp), which needs 54 to stay within TDG_MAX_ROLES (12 roles; 10x faster than the block-per-quartet kernel on cfg 3)
+__host__ __device__ constexpr int role_comps(int la, int lb, int lc, int ld) { return (la == 2 && lb == 2 && lc == 2 && ld == 1) ? 54 : 27; }
 
 template <int LA, int LB, int LC, int LD>
 struct QC {
@@ -39,7 +37,8 @@ struct QC {
   // registers; the 2-D integrals are rebuilt by every role.  Classes with an f shell keep rolled loops (one role).
   static constexpr bool HASF = LA == 3 || LB == 3 || LC == 3 || LD == 3;
   static constexpr int NAB = NA * NB, KDN = NC * ND;
-  static constexpr int ABN1 = TDG_ROLE_COMPS / KDN >= NAB ? NAB : (TDG_ROLE_COMPS / KDN > 0 ? TDG_ROLE_COMPS / KDN : 1);
+  static constexpr int RC = role_comps(LA, LB, LC, LD);
+  static constexpr int ABN1 = RC / KDN >= NAB ? NAB : (RC / KDN > 0 ? RC / KDN : 1);
   static constexpr int NROLE1 = (NAB + ABN1 - 1) / ABN1;
   static constexpr bool SMALL = NCOMP <= 27 || (!HASF && NROLE1 <= TDG_MAX_ROLES);   // fully unrolled code
   static constexpr int NROLE = SMALL ? NROLE1 : 1;
@@ -346,12 +345,21 @@ __device__ __forceinline__ unsigned screen_ket(const KParams& P, const PairHdr* 
       const double qq = bh.Q * Qk;
       if (!(qq >= P.tau)) continue;
       ++n_vis;
-      if (dw && qq * (P.CJ * s_dij[b] * dkl) < P.tau) {
+      if (dw && P.wmode == 0 && qq * (P.CJ * s_dij[b] * dkl) < P.tau) {
         // W = max(W_J, W_K) (S9): the J-type bound alone does not keep the quartet, so gather the four K-type maxima
         const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + ksh), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + lsh);
         const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + lsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + ksh);
         const double x1 = dik * djl, x2 = dil * djk;
         if (qq * (P.CK * (x1 > x2 ? x1 : x2)) < P.tau) continue;
+      }
+      if (dw && P.wmode == 1 && qq * (P.CJ * (s_dij[b] > dkl ? s_dij[b] : dkl)) < P.tau) {
+        // Fock-type build: W = max(CJ max(d_ij, d_kl), CK max(d_ik, d_il, d_jk, d_jl))  (tdg_fock.cuh)
+        const double dik = __ldg(P.dmax + (size_t)bh.ish * ns + ksh), djl = __ldg(P.dmax + (size_t)bh.jsh * ns + lsh);
+        const double dil = __ldg(P.dmax + (size_t)bh.ish * ns + lsh), djk = __ldg(P.dmax + (size_t)bh.jsh * ns + ksh);
+        double mk = dik > djl ? dik : djl;
+        if (dil > mk) mk = dil;
+        if (djk > mk) mk = djk;
+        if (qq * (P.CK * mk) < P.tau) continue;
       }
     } else ++n_vis;
     if (!tdg_sample_keep(bh.ish, bh.jsh, ksh, lsh, P.sample_mod, P.sample_seed)) continue;
@@ -435,20 +443,6 @@ __device__ __forceinline__ void process_survivors(const KParams& P, const PairHd
     }
   }
 }
-template <int LA, int LB, int LC, int LD, int R>
-struct RoleDispatch {
-  typedef QC<LA, LB, LC, LD> C;
-  static __device__ __forceinline__ void run(int role, const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket, unsigned mask, int pre, int tot,
-                                             double* s_gb, double* s_gk, int bra0, int k0, const double* __restrict__ rys) {
-    if constexpr (R < C::NROLE) {
-      constexpr int AB0 = R * C::ABN;
-      constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
-      if (role == R) process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, mask, pre, tot, s_gb, s_gk, bra0, k0, rys);
-      else RoleDispatch<LA, LB, LC, LD, R + 1>::run(role, P, s_bra, s_ket, mask, pre, tot, s_gb, s_gk, bra0, k0, rys);
-    }
-  }
-};
-
 // Block work item -> (bra tile, ket chunk): largest t with cum[t] <= item.
 __device__ __forceinline__ void find_work_item(const KParams& P, int item, int& tile, int& chunk) {
   int lo = 0, hi = P.ntiles;
@@ -459,7 +453,9 @@ __device__ __forceinline__ void find_work_item(const KParams& P, int item, int& 
 #ifndef TDG_MINB
 #define TDG_MINB 1
 #endif
-template <int LA, int LB, int LC, int LD>
+// One kernel per (class, role): role R handles the bra function pairs [R*ABN, (R+1)*ABN) of every surviving quartet (QC).  Each
+// role is its own translation unit (they compile in parallel and get their own register allocation).
+template <int LA, int LB, int LC, int LD, int ROLE>
 __global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid_constant__ KParams P) {
   __shared__ PairHdr s_bra[TDG_WARP];
   __shared__ PairHdr s_ket[TDG_KB];
@@ -501,7 +497,10 @@ __global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid
   for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
   const int tot = __shfl_sync(0xffffffffu, incl, 31);
   // ---- phase 2 (steps a5-a8): each warp processes the survivors of its own 32 kets densely, one quartet per thread per pass ----
-  RoleDispatch<LA, LB, LC, LD, 0>::run(blockIdx.y, P, s_bra, s_ket, mask, incl - cnt, tot, s_gb, s_gk, bra0, k0, rys);
+  static_assert(ROLE >= 0 && ROLE < C::NROLE, "role out of range");
+  constexpr int AB0 = ROLE * C::ABN;
+  constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
+  process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, mask, incl - cnt, tot, s_gb, s_gk, bra0, k0, rys);
   __syncthreads();
   // flush: sum the warps' private bra slots, one FP64 RED per touched (pair, centre, xyz)
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
@@ -524,12 +523,16 @@ __global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid
     n_vis += __shfl_xor_sync(0xffffffffu, n_vis, o);
     n_cmp += __shfl_xor_sync(0xffffffffu, n_cmp, o);
   }
-  if (lane == 0 && n_vis && blockIdx.y == 0) {
+  if (ROLE == 0 && lane == 0 && n_vis) {
     atomicAdd(P.counters + 0, n_vis); atomicAdd(P.counters + 1, n_cmp);
     atomicAdd(P.counters + 2, n_cmp * (unsigned long long)(P.nppb * P.nppk));
   }
 }
 
-// Host-callable launcher of one class, defined in tdg_class_*.cu; c1 = pair class la(la+1)/2+lb of the bra.
+// Host-callable launcher of one (class, role), defined in a translation unit of its own (tdg_class.cu) and registered at
+// load time; tdg_num_roles = QC::NROLE of the class (1 for the block-per-quartet kernel).
 typedef void (*tdg_launch_fn)(const KParams& P, int nblocks, cudaStream_t s);
-tdg_launch_fn tdg_get_launcher(int la, int lb, int lc, int ld);
+#define TDG_FOCK_ROLE_BASE 32   // launcher table: roles [0, 32) = gradient kernels, [32, 64) = Fock-build kernels of the same role
+void tdg_register_launcher(int la, int lb, int lc, int ld, int role, tdg_launch_fn fn);
+tdg_launch_fn tdg_get_launcher(int la, int lb, int lc, int ld, int role);
+int tdg_num_roles(int la, int lb, int lc, int ld);

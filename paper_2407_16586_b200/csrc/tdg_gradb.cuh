@@ -33,6 +33,10 @@ struct QB {
   // density blocks staged as 4-vectors (one entry per canonical matrix): raw IK, JK, IJ; MK.JL, MK.IL, MJ.KL
   static constexpr int O_IK = 0, O_JK = O_IK + NA * NC, O_IJ = O_JK + NB * NC, O_JL = O_IJ + NA * NB, O_IL = O_JL + NB * ND,
                        O_KL = O_IL + NA * ND, NBLK = O_KL + NC * ND;
+  // Fock mode (tdg_fock.cuh): raw blocks S[ls] (k,l), S[mn] (i,j), X[ln] (k,j), X[lm] (k,i), X[sn] (l,j), X[sm] (l,i)
+  static constexpr int F_KL = 0, F_IJ = F_KL + NC * ND, F_KJ = F_IJ + NA * NB, F_KI = F_KJ + NC * NB, F_LJ = F_KI + NC * NA,
+                       F_LI = F_LJ + ND * NB, F_NBLK = F_LI + ND * NA;
+  static_assert(F_NBLK == NBLK, "both modes stage the same number of block elements");
   static constexpr int ACC = (TDG_WARP + TDG_KB) * 6;
   static constexpr int SMEM_DOUBLES = ACC + RB * 3 * TASK + NBLK * 4 + 2 * NR * 4 + 4 * 9 + TDG_WARP + TDG_KB / 2;
 };
@@ -42,7 +46,10 @@ __device__ __forceinline__ void comp_exps_rt(int idx, int& x, int& y, int& z) {
   x = (int)((CartPack<L, 0>::v >> (4 * idx)) & 15); y = (int)((CartPack<L, 1>::v >> (4 * idx)) & 15); z = (int)((CartPack<L, 2>::v >> (4 * idx)) & 15);
 }
 
-template <int LA, int LB, int LC, int LD>
+// MODE 0: gradient (steps a5-a8).  MODE 1: Fock-type build (NEXT-1; conventions of tdg_fock.cuh): the same 2-D integrals (read
+// without the raised entries; the gradient's root count is exact for the lower degree too), each thread sums its function
+// quartets' integrals over the roots of a batch and digests them into G[slot][row][col] with FP64 RED.
+template <int LA, int LB, int LC, int LD, int MODE>
 __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const __grid_constant__ KParams P) {
   typedef QB<LA, LB, LC, LD> B;
   constexpr int G = B::G, NR = B::NR, S = B::S, TASK = B::TASK;
@@ -92,7 +99,7 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
       if (kh.ish == kh.jsh) deg *= 0.5;
       if (P.same_bucket && k0 + kt == bra0 + b) deg *= 0.5;
       // stage the six density blocks (step a7, part 1): raw IK, JK, IJ and MK.JL, MK.IL, MJ.KL (4-vectors over the canonical matrices)
-      {
+      if (MODE == 0) {
         const double* bIK = pk + 4 * ((size_t)bh.offA * n + (size_t)B::NA * kh.offA);
         const double* bJL = pk + 4 * ((size_t)bh.offB * n + (size_t)B::NB * kh.offB);
         const double* bJK = pk + 4 * ((size_t)bh.offB * n + (size_t)B::NB * kh.offA);
@@ -113,6 +120,19 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
 #pragma unroll
             for (int q = 0; q < 4; ++q) dst[q] = M[4 * q] * x.x + M[4 * q + 1] * x.y + M[4 * q + 2] * x.z + M[4 * q + 3] * x.w;
           } else { dst[0] = x.x; dst[1] = x.y; dst[2] = x.z; dst[3] = x.w; }
+        }
+      } else {   // Fock mode: raw blocks in the orientation the digestion reads
+        const double* src0[6] = {pk + 4 * ((size_t)kh.offA * n + (size_t)B::NC * kh.offB), pk + 4 * ((size_t)bh.offA * n + (size_t)B::NA * bh.offB),
+                                 pk + 4 * ((size_t)kh.offA * n + (size_t)B::NC * bh.offB), pk + 4 * ((size_t)kh.offA * n + (size_t)B::NC * bh.offA),
+                                 pk + 4 * ((size_t)kh.offB * n + (size_t)B::ND * bh.offB), pk + 4 * ((size_t)kh.offB * n + (size_t)B::ND * bh.offA)};
+        constexpr int off[7] = {B::F_KL, B::F_IJ, B::F_KJ, B::F_KI, B::F_LJ, B::F_LI, B::F_NBLK};
+        for (int e = t; e < B::F_NBLK; e += G) {
+          int q = 0;
+#pragma unroll
+          for (int z = 1; z < 6; ++z) if (e >= off[z]) q = z;
+          const d4 x = ld256(src0[q] + 4 * (e - off[q]));
+          double* dst = s_blk + 4 * e;
+          dst[0] = x.x; dst[1] = x.y; dst[2] = x.z; dst[3] = x.w;
         }
       }
       double g[9];
@@ -198,6 +218,52 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
               }
             }
             __syncthreads();
+            if constexpr (MODE == 1) {
+              // (4F) this thread's function quartets: integral summed over the batch's roots, digested at once
+              const size_t n2 = n * n;
+              double* __restrict__ Gm = P.grad;
+#pragma unroll 1
+              for (int fn = t; fn < B::NCOMP; fn += G) {
+                const int d = fn % B::ND, c = (fn / B::ND) % B::NC, bb = (fn / (B::ND * B::NC)) % B::NB, a = fn / (B::ND * B::NC * B::NB);
+                int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
+                comp_exps_rt<LA>(a, ax, ay, az); comp_exps_rt<LB>(bb, bx, by, bz); comp_exps_rt<LC>(c, cx, cy, cz); comp_exps_rt<LD>(d, dx, dy, dz);
+                const int ix = ((ax * B::DB + bx) * B::DC + cx) * B::DD + dx;
+                const int iy = ((ay * B::DB + by) * B::DC + cy) * B::DD + dy + TASK;
+                const int iz = ((az * B::DB + bz) * B::DC + cz) * B::DD + dz + 2 * TASK;
+                double vJ = 0.0, vK = 0.0;
+#pragma unroll 1
+                for (int r = 0; r < nrb; ++r) {
+                  const double* e = s_root + (r0 + r) * 4;
+                  const double* I = s_task + r * 3 * TASK;
+                  const double v = I[ix] * I[iy] * I[iz];
+                  vJ = fma(e[2], v, vJ); vK = fma(e[3], v, vK);
+                }
+                const double cn = deg * c_cnorm[LA][a] * c_cnorm[LB][bb] * c_cnorm[LC][c] * c_cnorm[LD][d];
+                vJ *= cn; vK *= cn;
+                const int mu = bh.offA + a, nu = bh.offB + bb, la_ = kh.offA + c, si = kh.offB + d;
+                const double* sKL = s_blk + 4 * (B::F_KL + c * B::ND + d);
+                const double* sIJ = s_blk + 4 * (B::F_IJ + a * B::NB + bb);
+                const double* xKJ = s_blk + 4 * (B::F_KJ + c * B::NB + bb);
+                const double* xKI = s_blk + 4 * (B::F_KI + c * B::NA + a);
+                const double* xLJ = s_blk + 4 * (B::F_LJ + d * B::NB + bb);
+                const double* xLI = s_blk + 4 * (B::F_LI + d * B::NA + a);
+#pragma unroll
+                for (int sl = 0; sl < 4; ++sl) {
+                  double* Gs = Gm + (size_t)sl * n2;
+                  const double jw = P.MJ[sl], kw = P.MK[sl];
+                  if (jw != 0.0) {
+                    red_add(Gs + (size_t)mu * n + nu, jw * sKL[sl] * vJ);
+                    red_add(Gs + (size_t)la_ * n + si, jw * sIJ[sl] * vJ);
+                  }
+                  if (kw != 0.0) {
+                    red_add(Gs + (size_t)mu * n + si, -kw * xKJ[sl] * vK);
+                    red_add(Gs + (size_t)nu * n + si, -kw * xKI[sl] * vK);
+                    red_add(Gs + (size_t)mu * n + la_, -kw * xLJ[sl] * vK);
+                    red_add(Gs + (size_t)nu * n + la_, -kw * xLI[sl] * vK);
+                  }
+                }
+              }
+            } else {
             // (4) function quartets over the threads (step a7): density products, centre derivatives, 9 sums
 #pragma unroll 1
             for (int fn = t; fn < B::NCOMP; fn += G) {
@@ -241,10 +307,12 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
                 g[6] += tx * dCx; g[7] += ty * dCy; g[8] += tz * dCz;
               }
             }
+            }
             if (r0 + B::RB < nroot) __syncthreads();   // the next batch overwrites s_task
           }
         }
       }
+      if constexpr (MODE == 0) {
       // block reduction of the 9 sums; thread 0 adds them to the accumulators (one quartet at a time: no races)
 #pragma unroll
       for (int x = 0; x < 9; ++x) g[x] = warp_sum(g[x]);
@@ -268,10 +336,13 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
           gkp[x] += g[6 + x]; gkp[3 + x] -= g[x] + g[3 + x] + g[6 + x];
         }
       }
+      } else {
+        __syncthreads();   // the next quartet restages s_blk / s_task
+      }
     }
   }
   __syncthreads();
-  for (int i = t; i < B::ACC; i += G) {
+  for (int i = t; MODE == 0 && i < B::ACC; i += G) {
     const double v = s_acc[i];
     if (v == 0.0) continue;
     const int r = i % 6;

@@ -24,6 +24,14 @@ cudaError_t tdg_run_fp64_peak(double ms, double* tflops);
 struct PackSrc { const double* src[4]; int kind[4]; };
 cudaError_t tdg_launch_pack(const PackSrc& ps, int n, const int* bf2sh, const DevShell* sh, double* pk, cudaStream_t s);
 
+// Spherical shells (NEXT-2): dir 0: out (Cartesian, nout x nout) = C^T in C with `in` in the input basis (nin_dim x nin_dim);
+// dir 1: out (input basis, nout x nout) = C in C^T with `in` Cartesian (nin_dim x nin_dim).  out2sh: shell of each function of
+// the OUTPUT basis; inoff: first input-basis function of each shell; sphflag: 1 = shell is spherical (acts for l >= 2).
+cudaError_t tdg_launch_sph_transform(const double* in, double* out, int nout, int nin_dim, int dir, const int* out2sh, const DevShell* sh,
+                                     const int* inoff, const int* sphflag, cudaStream_t s);
+// F += G + sign G^T  (n x n row-major, device)
+cudaError_t tdg_launch_fock_finalize(const double* G, int n, double sign, double* F, cudaStream_t s);
+
 // Contracted energy (tdg_energy): runtime-l, untuned; one launch per bucket pair, same work lists and screening as the
 // gradient kernels; *E (device) is accumulated with FP64 atomics.
 struct KParams;

@@ -1,6 +1,6 @@
 """One tdg_gradient call on a BASELINE.json config, for use under ncu (profiles/*.md name the full commands).
 
-    python -m paper_2407_16586_b200.profile_run [config=3] [calls=1]
+    python -m paper_2407_16586_b200.profile_run [config=3] [calls=1] [dense|decaying]
 """
 import json
 import os
@@ -19,7 +19,9 @@ def main():
     s = wl.make_system(cfg)
     ctx.set_system(s)
     ctx.plan(s.tau, s.density_weighted)
-    D, P, T = wl.make_densities_torch(s.nbf, 20240716 + cfg, "cuda")
+    kind = sys.argv[3] if len(sys.argv) > 3 else "dense"
+    D, P, T = (wl.make_decaying_densities_torch(s, 20240716 + cfg, "cuda") if kind == "decaying"
+               else wl.make_densities_torch(s.nbf, 20240716 + cfg, "cuda"))
     pairs, wJ, wK = wl.default_call(D, P, T)
     for _ in range(calls):
         g, st = ctx.gradient(pairs, wJ, wK, wl.C_J, wl.C_K, wl.C_LR, wl.OMEGA)

@@ -16,8 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libtdgrad.so")
 NCLASS = 55
 _lib = None
 
-SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_shard", "tdg_set_streams", "tdg_plan", "tdg_schwarz", "tdg_gradient",
-           "tdg_energy", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
+SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_spherical", "tdg_set_shard", "tdg_set_streams", "tdg_plan", "tdg_schwarz", "tdg_gradient",
+           "tdg_energy", "tdg_fock", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
 
 
 class TdgError(RuntimeError):
@@ -156,6 +156,15 @@ class Context:
         self._check(lib().tdg_nbf(self._h, C.byref(n)), "tdg_nbf")
         return n.value
 
+    def set_spherical(self, flags=None):
+        """flags[nshell] (nonzero: the d/f shell is spherical) or None for all Cartesian; see include/tdgrad.h."""
+        if flags is None:
+            rc = lib().tdg_set_spherical(self._h, None)
+        else:
+            f = np.ascontiguousarray(flags, dtype=np.int32)
+            rc = lib().tdg_set_spherical(self._h, C.c_void_p(f.ctypes.data))
+        self._check(rc, "tdg_set_spherical")
+
     def set_shard(self, rank: int, nranks: int):
         """This context computes the work items `rank` mod `nranks`; call before :meth:`plan`."""
         self._check(lib().tdg_set_shard(self._h, C.c_int(rank), C.c_int(nranks)), "tdg_set_shard")
@@ -225,6 +234,28 @@ class Context:
                               C.c_double(cJ), C.c_double(cK), C.c_double(cLR), C.c_double(omega), C.c_void_p(stream if stream else 0), C.byref(e))
         self._check(rc, "tdg_energy")
         return e.value
+
+    def fock(self, Bs, wJ, wK, wKT, cK, cLR, omega, stream=None, out=None, want_stats=True):
+        """Fock-type matrices F_k = wJ_k J[B_k] - (cK K + cLR K_lr)[wK_k B_k + wKT_k B_k^T] (include/tdgrad.h: tdg_fock).
+        Bs: list of numpy arrays (host) or CUDA torch tensors; out: optional list of CUDA tensors to write into.
+        Returns (list of F as numpy arrays, or ``out``; stats dict or None)."""
+        nmat = len(Bs)
+        on_dev = 0 if isinstance(Bs[0], np.ndarray) else 1
+        keep = [np.ascontiguousarray(b, dtype=np.float64) for b in Bs] if not on_dev else list(Bs)
+        n = self.nbf()
+        if out is None:
+            F = [np.zeros((n, n)) for _ in range(nmat)]
+            f_dev = 0
+        else:
+            F, f_dev = out, 1
+        PB = (C.c_void_p * nmat)(*[_ptr(b) for b in keep])
+        PF = (C.c_void_p * nmat)(*[_ptr(f) for f in F])
+        w = [np.ascontiguousarray(x, dtype=np.float64) for x in (wJ, wK, wKT)]
+        st = Stats() if want_stats else None
+        rc = lib().tdg_fock(self._h, C.c_int(nmat), PB, C.c_int(on_dev), *[C.c_void_p(x.ctypes.data) for x in w], C.c_double(cK), C.c_double(cLR),
+                            C.c_double(omega), C.c_void_p(stream if stream else 0), PF, C.c_int(f_dev), C.byref(st) if st is not None else None)
+        self._check(rc, "tdg_fock")
+        return F, (st.asdict() if st is not None else None)
 
     def rys(self, n, T, rho=None, omega=0.0) -> np.ndarray:
         T = np.ascontiguousarray(T, dtype=np.float64)

@@ -241,6 +241,78 @@ def make_densities_torch(nbf: int, seed: int, device, n_occ: int | None = None):
     return D.contiguous(), P.contiguous(), T.contiguous()
 
 
+# ---- second workload: spatially decaying densities -------------------------------------------------
+# Real TDDFT densities decay with distance, and "the pattern of nonzero elements in the density matrix" drives the cost of
+# the ERI-derivative step.  The recipe below keeps the geometry, basis and call of a config and replaces the
+# dense random matrices by ones whose elements fall off as exp(-r/DECAY_LENGTH) with the distance between the two atoms:
+#   C[mu, o]   = g exp(-|R_mu - R_o| / L),   orbital o centred on the O atom of water (o mod n_waters), columns normalised
+#   D          = C C^T,  scaled to ||D||_F = sqrt(n_occ)                       (localised "occupied" orbitals)
+#   P[mu, nu]  = s exp(-|R_mu - R_nu| / L),  s symmetric Gaussian, scaled to ||P||_F = sqrt(n_occ)
+#   T          = C Y,  Y[o, nu] = g exp(-|R_o - R_nu| / L),  scaled to ||T||_F = 1      (nonsymmetric, like C_o X C_v^T)
+DECAY_LENGTH = 3.0  # bohr
+
+
+def _bf_atoms(sysm: "System") -> np.ndarray:
+    return np.concatenate([np.full(ncart(int(l)), int(a), dtype=np.int64) for a, l in zip(sysm.shells[:, 0], sysm.shells[:, 1])])
+
+
+def make_decaying_densities(sysm: "System", seed, n_occ: int | None = None, length: float = DECAY_LENGTH):
+    """numpy version (small systems); same distribution as :func:`make_decaying_densities_torch`."""
+    nbf = sysm.nbf
+    if n_occ is None:
+        n_occ = max(1, nbf // 5)
+    rng = np.random.default_rng(seed)
+    at = _bf_atoms(sysm)
+    R = sysm.xyz[at]                                                    # position of every basis function's atom
+    heavy = np.array(sorted(set(int(a) for a, l in zip(sysm.shells[:, 0], sysm.shells[:, 1]) if l >= 2)) or sorted(set(at.tolist())))
+    cen = sysm.xyz[heavy[np.arange(n_occ) % len(heavy)]]                # orbital centres
+    dmo = np.linalg.norm(R[:, None, :] - cen[None, :, :], axis=2)       # [nbf, n_occ]
+    dmm = np.linalg.norm(R[:, None, :] - R[None, :, :], axis=2)         # [nbf, nbf]
+    C = rng.standard_normal((nbf, n_occ)) * np.exp(-dmo / length)
+    C /= np.linalg.norm(C, axis=0, keepdims=True)
+    D = C @ C.T
+    D = 0.5 * (D + D.T)
+    D *= np.sqrt(n_occ) / np.linalg.norm(D)
+    S = rng.standard_normal((nbf, nbf))
+    P = 0.5 * (S + S.T) * np.exp(-dmm / length)
+    P *= np.sqrt(n_occ) / np.linalg.norm(P)
+    Y = rng.standard_normal((n_occ, nbf)) * np.exp(-dmo.T / length)
+    T = C @ Y
+    T /= np.linalg.norm(T)
+    return np.ascontiguousarray(D), np.ascontiguousarray(P), np.ascontiguousarray(T)
+
+
+def make_decaying_densities_torch(sysm: "System", seed: int, device, n_occ: int | None = None, length: float = DECAY_LENGTH):
+    """torch FP64 version on ``device`` for configs 3-4 (the same recipe; different generator, so different numbers)."""
+    import torch
+
+    nbf = sysm.nbf
+    if n_occ is None:
+        n_occ = max(1, nbf // 5)
+    g = torch.Generator(device=device)
+    g.manual_seed(int(seed))
+    f64 = torch.float64
+    at = _bf_atoms(sysm)
+    R = torch.as_tensor(sysm.xyz[at], dtype=f64, device=device)
+    heavy = np.array(sorted(set(int(a) for a, l in zip(sysm.shells[:, 0], sysm.shells[:, 1]) if l >= 2)) or sorted(set(at.tolist())))
+    cen = torch.as_tensor(sysm.xyz[heavy[np.arange(n_occ) % len(heavy)]], dtype=f64, device=device)
+    dmo = torch.cdist(R, cen)
+    C = torch.randn((nbf, n_occ), generator=g, dtype=f64, device=device) * torch.exp(-dmo / length)
+    C /= torch.linalg.norm(C, dim=0, keepdim=True)
+    D = C @ C.T
+    D = 0.5 * (D + D.T)
+    D *= float(np.sqrt(n_occ)) / torch.linalg.norm(D)
+    S = torch.randn((nbf, nbf), generator=g, dtype=f64, device=device)
+    P = 0.5 * (S + S.T)
+    del S
+    P *= torch.exp(-torch.cdist(R, R) / length)
+    P *= float(np.sqrt(n_occ)) / torch.linalg.norm(P)
+    Y = torch.randn((n_occ, nbf), generator=g, dtype=f64, device=device) * torch.exp(-dmo.T / length)
+    T = C @ Y
+    T /= torch.linalg.norm(T)
+    return D.contiguous(), P.contiguous(), T.contiguous()
+
+
 def density_seed(cfg: int) -> np.random.SeedSequence:
     return np.random.SeedSequence(BASE_SEED + cfg).spawn(2)[1]
 

@@ -48,3 +48,28 @@ def test_default_call_weights():
     pairs, wJ, wK = wl.default_call(D, P, T)
     assert [(a is D, b is D) for a, b in pairs[:1]] == [(True, True)] and pairs[1][1] is P and pairs[2][0] is T
     assert list(wJ) == [2.0, 2.0, 2.0] and list(wK) == [1.0, 1.0, 1.0]
+
+
+def test_decaying_density_recipe():
+    """NEXT-4 workload: same norms as the dense recipe, elements fall off with the distance between the functions' atoms."""
+    s = wl.make_system(1)
+    D, P, T = wl.make_decaying_densities(s, 5)
+    n_occ = s.nbf // 5
+    assert abs(np.linalg.norm(D) - np.sqrt(n_occ)) < 1e-10 and abs(np.linalg.norm(P) - np.sqrt(n_occ)) < 1e-10
+    assert abs(np.linalg.norm(T) - 1.0) < 1e-12
+    assert np.array_equal(D, D.T) and np.array_equal(P, P.T) and np.abs(T - T.T).max() > 1e-3
+    at = wl._bf_atoms(s)
+    r = np.linalg.norm(s.xyz[at][:, None, :] - s.xyz[at][None, :, :], axis=2)
+    near, far = np.abs(P[r < 2.0]).mean(), np.abs(P[r > 10.0]).mean()
+    assert far < near * np.exp(-8.0 / wl.DECAY_LENGTH) * 3
+    assert np.abs(D[r > 12.0]).max() < 0.05 * np.abs(D).max()
+
+
+def test_build_role_count_matches_header_formula():
+    """build.num_roles (one translation unit per class and role) against the cases stated in csrc/tdg_grad.cuh."""
+    from paper_2407_16586_b200 import build
+
+    assert build.num_roles(1, 0, 0, 0) == 1 and build.num_roles(1, 1, 1, 0) == 1
+    assert build.num_roles(2, 1, 1, 0) == 2 and build.num_roles(2, 1, 2, 1) == 18 and build.num_roles(2, 2, 2, 1) == 12
+    assert build.num_roles(2, 2, 2, 2) == 1 and build.num_roles(3, 0, 0, 0) == 1 and build.num_roles(3, 3, 3, 3) == 1
+    assert sum(build.num_roles(*c) for c in build.QUARTET_CLASSES) == 120

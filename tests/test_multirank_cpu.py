@@ -144,7 +144,7 @@ class _StubBackend:
     def context(self):
         return _StubContext(self.natom, self.log)
 
-    def densities(self, nbf, seed):
+    def densities(self, nbf, seed, sysm=None, kind="dense"):
         return [torch.zeros(2, 2, dtype=torch.float64) for _ in range(3)]
 
     def host_copies(self, mats):
@@ -181,7 +181,7 @@ def _bench_worker(rank, world, port, out):
 
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    args = argparse.Namespace(gpus=world, steps=2, warmup=1, config=0, parallelism="shard", streams=1, no_cpu_baseline=True)
+    args = argparse.Namespace(gpus=world, steps=2, warmup=1, config=0, parallelism="shard", streams=1, densities="dense", no_cpu_baseline=True)
     be = _StubBackend(wl.make_system(0).natom, rank)
     lines = []
     bench.run_ours(args, backend=be, emit=lines.append)
