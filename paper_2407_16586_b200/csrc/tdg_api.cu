@@ -14,6 +14,7 @@
 
 #define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
 #define TDG_MAX_STREAMS 8
+#define TDG_ROLE_STREAMS 6   // streams the roles of one class launch are spread over
 
 // Launchers register themselves at load time (one translation unit per class and role, tdg_class.cu).
 #define TDG_ROLE_SLOTS 64
@@ -76,6 +77,8 @@ struct tdg_ctx {
   int nstreams = 1;                  // tdg_set_streams: class launches are dealt over the caller's stream + nstreams-1 side streams
   cudaStream_t side[TDG_MAX_STREAMS - 1] = {};
   cudaEvent_t ev_fork = nullptr, ev_join[TDG_MAX_STREAMS - 1] = {};
+  cudaStream_t rstream[TDG_ROLE_STREAMS - 1] = {};   // role streams (created with the context)
+  cudaEvent_t ev_rfork = nullptr, ev_rjoin[TDG_ROLE_STREAMS - 1] = {};
   // per-call scratch
   double* d_grad = nullptr;
   double* d_dmax = nullptr;
@@ -136,6 +139,11 @@ extern "C" int tdg_create(tdg_ctx** out, int cuda_device) {
   if (!ctx) return TDG_ENOMEM;
   ctx->device = cuda_device;
   if (tdg_upload_rys_table(&ctx->d_rys) != cudaSuccess) { delete ctx; return TDG_ECUDA; }
+  bool ok = cudaEventCreateWithFlags(&ctx->ev_rfork, cudaEventDisableTiming) == cudaSuccess;
+  for (int i = 0; ok && i < TDG_ROLE_STREAMS - 1; ++i)
+    ok = cudaStreamCreateWithFlags(&ctx->rstream[i], cudaStreamNonBlocking) == cudaSuccess &&
+         cudaEventCreateWithFlags(&ctx->ev_rjoin[i], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) { tdg_destroy(ctx); return TDG_ECUDA; }
   *out = ctx;
   return TDG_OK;
 }
@@ -150,6 +158,11 @@ extern "C" int tdg_destroy(tdg_ctx* ctx) {
     if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
   }
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  for (int i = 0; i < TDG_ROLE_STREAMS - 1; ++i) {
+    if (ctx->rstream[i]) cudaStreamDestroy(ctx->rstream[i]);
+    if (ctx->ev_rjoin[i]) cudaEventDestroy(ctx->ev_rjoin[i]);
+  }
+  if (ctx->ev_rfork) cudaEventDestroy(ctx->ev_rfork);
   delete ctx;
   return TDG_OK;
 }
@@ -562,15 +575,24 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
       cudaStream_t ls = si == 0 ? st : ctx->side[si - 1];
       cudaEvent_t e0 = nullptr, e1 = nullptr;
       if (stats) { e0 = pool.get(); e1 = pool.get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, ls); }
-      if (d_E) CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, ls));
-      else
-        for (int role = 0; role < nrole; ++role) {   // the roles of a class are separate kernels (slices of the bra function pairs)
+      if (d_E) { CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, ls)); ++launches; }
+      else {
+        // the roles of a class are separate kernels (slices of the bra function pairs of the same quartets): run them side by
+        // side on the role streams, forked from and joined to the launch's stream, so they share the pair data in L2 and one tail
+        const int nrs = std::min(nrole, TDG_ROLE_STREAMS);
+        if (nrs > 1) {
+          CK(cudaEventRecord(ctx->ev_rfork, ls));
+          for (int i = 1; i < nrs; ++i) CK(cudaStreamWaitEvent(ctx->rstream[i - 1], ctx->ev_rfork, 0));
+        }
+        for (int role = 0; role < nrole; ++role) {
           tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb, role);
           if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
-          fn(P, W.nblocks, ls);
+          const int ri = role % nrs;
+          fn(P, W.nblocks, ri == 0 ? ls : ctx->rstream[ri - 1]);
           ++launches;
         }
-      if (d_E) ++launches;
+        for (int i = 1; i < nrs; ++i) { CK(cudaEventRecord(ctx->ev_rjoin[i - 1], ctx->rstream[i - 1])); CK(cudaStreamWaitEvent(ls, ctx->ev_rjoin[i - 1], 0)); }
+      }
       if (stats) { cudaEventRecord(e1, ls); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(W.cls); }
     }
     if (nstr > 1)

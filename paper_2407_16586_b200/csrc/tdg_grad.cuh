@@ -364,8 +364,9 @@ __device__ __forceinline__ unsigned screen_ket(const KParams& P, const PairHdr* 
     } else ++n_vis;
     if (!tdg_sample_keep(bh.ish, bh.jsh, ksh, lsh, P.sample_mod, P.sample_seed)) continue;
     ++n_cmp;
-    // all four shells on one atom: the four centre derivatives sum to zero on that atom (reading S11)
-    if (ket_one && bh.atomA == bh.atomB && bh.atomA == kh.atomA) continue;
+    // all four shells on one atom: the four centre derivatives sum to zero on that atom (reading S11); the undifferentiated
+    // integrals of the Fock-type build (wmode 1) do not vanish
+    if (P.wmode == 0 && ket_one && bh.atomA == bh.atomB && bh.atomA == kh.atomA) continue;
     mask |= 1u << b;
   }
   return mask;
