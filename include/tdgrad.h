@@ -109,9 +109,10 @@ int tdg_plan(tdg_ctx* ctx, const tdg_options* opt);
  * Invalidates the plan when the shard changes.  TDG_EINVAL unless 0 <= rank < nranks. */
 int tdg_set_shard(tdg_ctx* ctx, int rank, int nranks);
 
-/* Class launches of one tdg_gradient call are independent; with nstreams > 1 they are dealt over the caller's stream and
- * nstreams-1 internal streams that fork from / join it by events, so the call stays stream-ordered for the caller.
- * Per-class times in tdg_stats then overlap (their sum exceeds ms_total).  1 <= nstreams <= 8; default 1. */
+/* The kernel launches of one quartet class (one per bucket pair and role) are independent of each other; they are dealt over the
+ * caller's stream and nstreams-1 internal streams that fork from it before the class and join it after (events), so tails and
+ * under-filled launches overlap while the call stays stream-ordered for the caller and tdg_stats.ms_by_class stays the wall time
+ * of each class.  1 <= nstreams <= 8; default 6; 1 = strictly serial launches. */
 int tdg_set_streams(tdg_ctx* ctx, int nstreams);
 
 /* Schwarz bounds of the current system: Q[nshell][nshell] to a HOST buffer (for tests/diagnostics). */

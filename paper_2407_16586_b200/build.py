@@ -33,7 +33,7 @@ def num_roles(la: int, lb: int, lc: int, ld: int) -> int:
     nab, kdn = ncart(la) * ncart(lb), ncart(lc) * ncart(ld)
     abn1 = nab if rc // kdn >= nab else max(rc // kdn, 1)
     nrole1 = -(-nab // abn1)
-    small = nab * kdn <= 27 or (3 not in (la, lb, lc, ld) and nrole1 <= 18)
+    small = nab * kdn <= 27 or nrole1 <= (8 if 3 in (la, lb, lc, ld) else 18)
     return nrole1 if small else 1
 DEPS = {   # headers each source includes
     "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "rys_meta.inc"],

@@ -1,6 +1,8 @@
 // tdg_api.cu — C ABI of libtdgrad (include/tdgrad.h): context, host planner (steps a0-a2), density preparation
 // and per-class launches (a3-a9).  No CPU arithmetic fallback: all integrals are evaluated by the CUDA kernels.
 #include <algorithm>
+#include <atomic>
+#include <thread>
 #include <cmath>
 #include <cstring>
 #include <map>
@@ -14,7 +16,7 @@
 
 #define PCLS(la, lb) ((la) * ((la) + 1) / 2 + (lb))
 #define TDG_MAX_STREAMS 8
-#define TDG_ROLE_STREAMS 6   // streams the roles of one class launch are spread over
+#define TDG_DEFAULT_STREAMS 6
 
 // Launchers register themselves at load time (one translation unit per class and role, tdg_class.cu).
 #define TDG_ROLE_SLOTS 64
@@ -72,13 +74,12 @@ struct tdg_ctx {
   tdg_options opt{};
   std::vector<Bucket> buckets;
   std::vector<Work> work;
+  char* d_arena = nullptr;
   int64_t pairs_total = 0, pairs_kept = 0;
   int shard_rank = 0, shard_n = 1;   // tdg_set_shard: this context owns every shard_n-th (launch, bra tile) work item
-  int nstreams = 1;                  // tdg_set_streams: class launches are dealt over the caller's stream + nstreams-1 side streams
+  int nstreams = 1;                  // tdg_set_streams: the launches of ONE class are dealt over the caller's stream + nstreams-1 side streams
   cudaStream_t side[TDG_MAX_STREAMS - 1] = {};
   cudaEvent_t ev_fork = nullptr, ev_join[TDG_MAX_STREAMS - 1] = {};
-  cudaStream_t rstream[TDG_ROLE_STREAMS - 1] = {};   // role streams (created with the context)
-  cudaEvent_t ev_rfork = nullptr, ev_rjoin[TDG_ROLE_STREAMS - 1] = {};
   // per-call scratch
   double* d_grad = nullptr;
   double* d_dmax = nullptr;
@@ -99,8 +100,7 @@ static int fail_cuda(tdg_ctx* c, cudaError_t e, const char* where) {
   } while (0)
 
 static void free_plan(tdg_ctx* c) {
-  for (auto& b : c->buckets) { cudaFree(b.d_hdr); cudaFree(b.d_prim); }
-  for (auto& w : c->work) cudaFree(w.d_cum);
+  cudaFree(c->d_arena); c->d_arena = nullptr;   // bucket headers, primitive-pair records and work lists live in one allocation
   c->buckets.clear(); c->work.clear();
   c->planned = false;
 }
@@ -139,12 +139,8 @@ extern "C" int tdg_create(tdg_ctx** out, int cuda_device) {
   if (!ctx) return TDG_ENOMEM;
   ctx->device = cuda_device;
   if (tdg_upload_rys_table(&ctx->d_rys) != cudaSuccess) { delete ctx; return TDG_ECUDA; }
-  bool ok = cudaEventCreateWithFlags(&ctx->ev_rfork, cudaEventDisableTiming) == cudaSuccess;
-  for (int i = 0; ok && i < TDG_ROLE_STREAMS - 1; ++i)
-    ok = cudaStreamCreateWithFlags(&ctx->rstream[i], cudaStreamNonBlocking) == cudaSuccess &&
-         cudaEventCreateWithFlags(&ctx->ev_rjoin[i], cudaEventDisableTiming) == cudaSuccess;
-  if (!ok) { tdg_destroy(ctx); return TDG_ECUDA; }
   *out = ctx;
+  if (tdg_set_streams(ctx, TDG_DEFAULT_STREAMS) != TDG_OK) { *out = nullptr; tdg_destroy(ctx); return TDG_ECUDA; }
   return TDG_OK;
 }
 
@@ -158,11 +154,6 @@ extern "C" int tdg_destroy(tdg_ctx* ctx) {
     if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
   }
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-  for (int i = 0; i < TDG_ROLE_STREAMS - 1; ++i) {
-    if (ctx->rstream[i]) cudaStreamDestroy(ctx->rstream[i]);
-    if (ctx->ev_rjoin[i]) cudaEventDestroy(ctx->ev_rjoin[i]);
-  }
-  if (ctx->ev_rfork) cudaEventDestroy(ctx->ev_rfork);
   delete ctx;
   return TDG_OK;
 }
@@ -320,59 +311,75 @@ extern "C" int tdg_plan(tdg_ctx* ctx, const tdg_options* opt) {
     for (double q : Q) if (q > Qmax) Qmax = q;
   }
   struct HP { int i, j; double Q; };
-  std::map<std::tuple<int, int, int>, std::vector<HP>> groups;  // (pair class, npp) -> pairs; ordered
+  // buckets keyed by (pair class, primitive-pair count); a shell's "type" (l, nprim) decides the key, so the pair loop below
+  // only indexes a small table (the loop runs over all nshell^2/2 pairs: 4.7e6 at cfg 3, 7.5e7 at cfg 4)
+  std::vector<std::pair<int, int>> types;          // distinct (l, nprim)
+  std::vector<int> type_of(ns);
+  for (int i = 0; i < ns; ++i) {
+    const std::pair<int, int> t(ctx->shells[i].l, ctx->shells[i].nprim);
+    size_t k = 0;
+    while (k < types.size() && types[k] != t) ++k;
+    if (k == types.size()) types.push_back(t);
+    type_of[i] = (int)k;
+  }
+  const int nt = (int)types.size();
+  std::map<std::pair<int, int>, int> key2group;    // (pair class, npp) -> group, ordered: bucket order = key order
+  std::vector<int> tab((size_t)nt * nt, -1);
+  for (int a = 0; a < nt; ++a)
+    for (int b = 0; b < nt; ++b) {
+      const int la = std::max(types[a].first, types[b].first), lb = std::min(types[a].first, types[b].first);
+      key2group[{PCLS(la, lb), types[a].second * types[b].second}] = 0;
+    }
+  {
+    int g = 0;
+    for (auto& kv : key2group) kv.second = g++;
+    for (int a = 0; a < nt; ++a)
+      for (int b = 0; b < nt; ++b) {
+        const int la = std::max(types[a].first, types[b].first), lb = std::min(types[a].first, types[b].first);
+        tab[(size_t)a * nt + b] = key2group[{PCLS(la, lb), types[a].second * types[b].second}];
+      }
+  }
   ctx->pairs_total = (int64_t)ns * (ns + 1) / 2;
   ctx->pairs_kept = 0;
-  for (int i = 0; i < ns; ++i)
-    for (int j = 0; j <= i; ++j) {
-      double q = 1.0;
-      if (tau > 0.0) { q = Q[(size_t)i * ns + j]; if (!(q * Qmax >= tau)) continue; }
-      int a = i, b = j;   // orient: higher l first; ties keep i (the larger index) first
-      if (ctx->shells[a].l < ctx->shells[b].l) std::swap(a, b);
-      const int la = ctx->shells[a].l, lb = ctx->shells[b].l;
-      groups[std::make_tuple(PCLS(la, lb), ctx->shells[a].nprim * ctx->shells[b].nprim, 0)].push_back(HP{a, b, q});
-      ++ctx->pairs_kept;
-    }
   try {
-    for (auto& kv : groups) {
-      auto& v = kv.second;
+    std::vector<std::vector<HP>> groups(key2group.size());
+    for (int i = 0; i < ns; ++i) {
+      const int ti = type_of[i], li = ctx->shells[i].l;
+      const double* Qi = tau > 0.0 ? &Q[(size_t)i * ns] : nullptr;
+      for (int j = 0; j <= i; ++j) {
+        double q = 1.0;
+        if (Qi) { q = Qi[j]; if (!(q * Qmax >= tau)) continue; }
+        // orient: higher l first; ties keep i (the larger index) first
+        if (li < ctx->shells[j].l) groups[tab[(size_t)ti * nt + type_of[j]]].push_back(HP{j, i, q});
+        else groups[tab[(size_t)ti * nt + type_of[j]]].push_back(HP{i, j, q});
+        ++ctx->pairs_kept;
+      }
+    }
+    // sort every bucket by Q descending; lay out headers, primitive-pair records and work lists in ONE host
+    // arena, uploaded with one allocation and one copy (the plan is rebuilt at every geometry: allocator calls add up)
+    auto align16 = [](size_t x) { return (x + 255) & ~(size_t)255; };   // 256-bit loads of the records need 32 bytes; 256 keeps every array on its own line
+    size_t bytes = 0;
+    std::vector<size_t> off_hdr, off_prim;
+    for (auto& kv : key2group) {
+      auto& v = groups[kv.second];
+      if (v.empty()) continue;
       std::sort(v.begin(), v.end(), [](const HP& x, const HP& y) {
         if (x.Q != y.Q) return x.Q > y.Q;
         if (x.i != y.i) return x.i < y.i;
         return x.j < y.j;
       });
       Bucket B;
-      B.la = ctx->shells[v[0].i].l; B.lb = ctx->shells[v[0].j].l; B.npp = std::get<1>(kv.first); B.n = (int)v.size();
-      std::vector<PairHdr> hdr(v.size());
-      std::vector<double> prim(v.size() * (size_t)B.npp * TDG_PRIM_STRIDE, 0.0);
+      B.la = ctx->shells[v[0].i].l; B.lb = ctx->shells[v[0].j].l; B.npp = kv.first.second; B.n = (int)v.size();
       B.Q.resize(v.size());
-      for (size_t t = 0; t < v.size(); ++t) {
-        const DevShell& sa = ctx->shells[v[t].i]; const DevShell& sb = ctx->shells[v[t].j];
-        const double* A = &ctx->xyz[3 * sa.atom]; const double* Bc = &ctx->xyz[3 * sb.atom];
-        PairHdr& h = hdr[t];
-        double R2 = 0.0;
-        for (int d = 0; d < 3; ++d) { h.A[d] = A[d]; h.AB[d] = A[d] - Bc[d]; R2 += h.AB[d] * h.AB[d]; }
-        h.Q = v[t].Q; h.ish = v[t].i; h.jsh = v[t].j; h.atomA = sa.atom; h.atomB = sb.atom; h.offA = sa.bf_off; h.offB = sb.bf_off;
-        B.Q[t] = v[t].Q;
-        double* pp = &prim[t * (size_t)B.npp * TDG_PRIM_STRIDE];
-        for (int ka = 0; ka < sa.nprim; ++ka)
-          for (int kb = 0; kb < sb.nprim; ++kb) {
-            const double a = ctx->exps[sa.prim_off + ka], b = ctx->exps[sb.prim_off + kb], p = a + b;
-            double* r = pp + (size_t)(ka * sb.nprim + kb) * TDG_PRIM_STRIDE;
-            r[0] = p;
-            for (int d = 0; d < 3; ++d) r[1 + d] = (a * A[d] + b * Bc[d]) / p;
-            r[4] = ctx->cn[sa.prim_off + ka] * ctx->cn[sb.prim_off + kb] * std::exp(-a * b / p * R2) / p;
-            r[5] = a; r[6] = b; r[7] = 1.0 / p;
-          }
-      }
-      CK(cudaMalloc(&B.d_hdr, sizeof(PairHdr) * hdr.size()));
-      CK(cudaMalloc(&B.d_prim, sizeof(double) * prim.size()));
-      CK(cudaMemcpy(B.d_hdr, hdr.data(), sizeof(PairHdr) * hdr.size(), cudaMemcpyHostToDevice));
-      CK(cudaMemcpy(B.d_prim, prim.data(), sizeof(double) * prim.size(), cudaMemcpyHostToDevice));
+      for (size_t t = 0; t < v.size(); ++t) B.Q[t] = v[t].Q;
+      off_hdr.push_back(bytes); bytes = align16(bytes + sizeof(PairHdr) * v.size());
+      off_prim.push_back(bytes); bytes = align16(bytes + sizeof(double) * v.size() * (size_t)B.npp * TDG_PRIM_STRIDE);
       ctx->buckets.push_back(std::move(B));
     }
     // work lists: bucket b1 >= b2 (bucket order = (pair class, npp) ascending, so bra class >= ket class)
     const int nb = (int)ctx->buckets.size();
+    std::vector<std::vector<int>> cums;
+    std::vector<size_t> off_cum;
     int64_t item = 0;   // running index of non-empty (launch, bra tile) work items, dealt round-robin over the ranks
     for (int b1 = 0; b1 < nb; ++b1)
       for (int b2 = 0; b2 <= b1; ++b2) {
@@ -394,10 +401,65 @@ extern "C" int tdg_plan(tdg_ctx* ctx, const tdg_options* opt) {
         W.b1 = b1; W.b2 = b2; W.ntiles = ntiles; W.nblocks = cum[ntiles];
         const int c1 = PCLS(X.la, X.lb), c2 = PCLS(Y.la, Y.lb);
         W.cls = c1 * (c1 + 1) / 2 + c2;
-        CK(cudaMalloc(&W.d_cum, sizeof(int) * cum.size()));
-        CK(cudaMemcpy(W.d_cum, cum.data(), sizeof(int) * cum.size(), cudaMemcpyHostToDevice));
+        off_cum.push_back(bytes); bytes = align16(bytes + sizeof(int) * cum.size());
+        cums.push_back(std::move(cum));
         ctx->work.push_back(W);
       }
+    // fill the arena (bucket by bucket on a few host threads: exp() per primitive pair) and upload it
+    std::vector<char> host(bytes);
+    {
+      std::vector<std::thread> pool;
+      std::atomic<int> next(0);
+      const int nthr = std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
+      std::vector<const std::vector<HP>*> bucket_pairs;
+      for (auto& kv : key2group) if (!groups[kv.second].empty()) bucket_pairs.push_back(&groups[kv.second]);
+      // work units: (bucket, slice of 4096 pairs)
+      struct Unit { int b; size_t t0, t1; };
+      std::vector<Unit> units;
+      for (int b = 0; b < nb; ++b)
+        for (size_t t0 = 0; t0 < bucket_pairs[b]->size(); t0 += 4096) units.push_back(Unit{b, t0, std::min(bucket_pairs[b]->size(), t0 + 4096)});
+      auto fill = [&]() {
+        for (;;) {
+          const int u = next.fetch_add(1);
+          if (u >= (int)units.size()) return;
+          const Bucket& B = ctx->buckets[units[u].b];
+          const std::vector<HP>& v = *bucket_pairs[units[u].b];
+          PairHdr* hdr = reinterpret_cast<PairHdr*>(host.data() + off_hdr[units[u].b]);
+          double* prim = reinterpret_cast<double*>(host.data() + off_prim[units[u].b]);
+          for (size_t t = units[u].t0; t < units[u].t1; ++t) {
+            const DevShell& sa = ctx->shells[v[t].i]; const DevShell& sb = ctx->shells[v[t].j];
+            const double* A = &ctx->xyz[3 * sa.atom]; const double* Bc = &ctx->xyz[3 * sb.atom];
+            PairHdr& h = hdr[t];
+            double R2 = 0.0;
+            for (int d = 0; d < 3; ++d) { h.A[d] = A[d]; h.AB[d] = A[d] - Bc[d]; R2 += h.AB[d] * h.AB[d]; }
+            h.Q = v[t].Q; h.ish = v[t].i; h.jsh = v[t].j; h.atomA = sa.atom; h.atomB = sb.atom; h.offA = sa.bf_off; h.offB = sb.bf_off;
+            double* pp = prim + t * (size_t)B.npp * TDG_PRIM_STRIDE;
+            for (int ka = 0; ka < sa.nprim; ++ka)
+              for (int kb = 0; kb < sb.nprim; ++kb) {
+                const double a = ctx->exps[sa.prim_off + ka], b = ctx->exps[sb.prim_off + kb], p = a + b;
+                double* r = pp + (size_t)(ka * sb.nprim + kb) * TDG_PRIM_STRIDE;
+                r[0] = p;
+                for (int d = 0; d < 3; ++d) r[1 + d] = (a * A[d] + b * Bc[d]) / p;
+                r[4] = ctx->cn[sa.prim_off + ka] * ctx->cn[sb.prim_off + kb] * std::exp(-a * b / p * R2) / p;
+                r[5] = a; r[6] = b; r[7] = 1.0 / p;
+              }
+          }
+        }
+      };
+      for (int t = 1; t < nthr; ++t) pool.emplace_back(fill);
+      fill();
+      for (auto& th : pool) th.join();
+    }
+    for (size_t w = 0; w < cums.size(); ++w) std::memcpy(host.data() + off_cum[w], cums[w].data(), sizeof(int) * cums[w].size());
+    if (bytes) {
+      CK(cudaMalloc(&ctx->d_arena, bytes));
+      CK(cudaMemcpy(ctx->d_arena, host.data(), bytes, cudaMemcpyHostToDevice));
+    }
+    for (int b = 0; b < nb; ++b) {
+      ctx->buckets[b].d_hdr = reinterpret_cast<PairHdr*>(ctx->d_arena + off_hdr[b]);
+      ctx->buckets[b].d_prim = reinterpret_cast<double*>(ctx->d_arena + off_prim[b]);
+    }
+    for (size_t w = 0; w < cums.size(); ++w) ctx->work[w].d_cum = reinterpret_cast<int*>(ctx->d_arena + off_cum[w]);
   } catch (const std::bad_alloc&) { free_plan(ctx); return TDG_ENOMEM; }
   const size_t need = ctx->work.size() * 3 + 3;
   if (need > ctx->counters_cap) {
@@ -450,6 +512,53 @@ static int to_device_cart(tdg_ctx* ctx, const double* M, int on_dev, cudaStream_
     src = cart;
   }
   *out = src;
+  return TDG_OK;
+}
+
+// The launches of one class (one kernel per role, one launch per bucket pair) are independent: they only add into the output
+// and into their own counters.  They are dealt over the caller's stream and nstreams-1 side streams that fork from it before
+// the class and join it after, so under-filled launches and tails overlap, roles run side by side, and the CUDA events around
+// the class (on the caller's stream) time exactly that class.  role_base: 0 gradient kernels, TDG_FOCK_ROLE_BASE Fock kernels.
+static int launch_classes(tdg_ctx* ctx, KParams& P, int role_base, double* d_E, bool count_here, cudaStream_t st, EventPool* pool,
+                          std::vector<cudaEvent_t>& evs, std::vector<int>& ev_cls, int& launches) {
+  const size_t nw = ctx->work.size();
+  const int nstr = d_E ? 1 : ctx->nstreams;
+  std::vector<size_t> order(nw);
+  for (size_t w = 0; w < nw; ++w) order[w] = w;
+  std::stable_sort(order.begin(), order.end(), [&](size_t x, size_t y) { return ctx->work[x].cls < ctx->work[y].cls; });
+  for (size_t g0 = 0; g0 < nw;) {
+    size_t g1 = g0;
+    while (g1 < nw && ctx->work[order[g1]].cls == ctx->work[order[g0]].cls) ++g1;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (pool) { e0 = pool->get(); e1 = pool->get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, st); }
+    if (nstr > 1) {
+      CK(cudaEventRecord(ctx->ev_fork, st));
+      for (int i = 0; i < nstr - 1; ++i) CK(cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
+    }
+    int unit = 0;
+    for (size_t gw = g0; gw < g1; ++gw) {
+      const size_t w = order[gw];
+      const Work& W = ctx->work[w];
+      const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
+      P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
+      P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
+      P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
+      P.counters = ctx->d_counters + 3 * (count_here ? w : nw);   // quartet counts come from the first pass only
+      if (d_E) { CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, st)); ++launches; continue; }
+      const int nrole = tdg_num_roles(X.la, X.lb, Y.la, Y.lb);
+      for (int role = 0; role < nrole; ++role) {   // the roles of a class are separate kernels (slices of the bra function pairs)
+        tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb, role + role_base);
+        if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
+        const int si = unit++ % nstr;
+        fn(P, W.nblocks, si == 0 ? st : ctx->side[si - 1]);
+        ++launches;
+      }
+    }
+    if (nstr > 1)
+      for (int i = 0; i < nstr - 1; ++i) { CK(cudaEventRecord(ctx->ev_join[i], ctx->side[i])); CK(cudaStreamWaitEvent(st, ctx->ev_join[i], 0)); }
+    if (pool) { cudaEventRecord(e1, st); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(ctx->work[order[g0]].cls); }
+    g0 = g1;
+  }
   return TDG_OK;
 }
 
@@ -537,7 +646,6 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
   int launches = 0;
   std::vector<cudaEvent_t> evs;   // (start, stop) per launch, on the launch's own stream
   std::vector<int> ev_cls;
-  const int nstr = d_E ? 1 : ctx->nstreams;
   for (size_t gi = 0; gi < groups.size(); ++gi) {
     const Group& G = groups[gi];
     PackSrc ps{};
@@ -557,46 +665,10 @@ static int run_contraction(tdg_ctx* ctx, int npair, const double* const* A, cons
         P.MK[4 * na + nb] += wk; P.MK[4 * nb + na] += wk;
       }
     }
-    // class launches are independent (they only add into grad and their own counters): deal them over the streams so
-    // that the under-filled tail of one launch overlaps the next; the side streams fork from and join the caller's
-    if (nstr > 1) {
-      CK(cudaEventRecord(ctx->ev_fork, st));
-      for (int i = 0; i < nstr - 1; ++i) CK(cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
+    {
+      const int rc_l = launch_classes(ctx, P, 0, d_E, gi == 0, st, stats ? &pool : nullptr, evs, ev_cls, launches);
+      if (rc_l) return rc_l;
     }
-    for (size_t w = 0; w < nw; ++w) {
-      const Work& W = ctx->work[w];
-      const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
-      const int nrole = d_E ? 1 : tdg_num_roles(X.la, X.lb, Y.la, Y.lb);
-      P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
-      P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
-      P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
-      P.counters = ctx->d_counters + 3 * (gi == 0 ? w : nw);   // quartet counts come from the first group only
-      const int si = (int)(w % (size_t)nstr);
-      cudaStream_t ls = si == 0 ? st : ctx->side[si - 1];
-      cudaEvent_t e0 = nullptr, e1 = nullptr;
-      if (stats) { e0 = pool.get(); e1 = pool.get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, ls); }
-      if (d_E) { CK(tdg_launch_energy(P, X.la, X.lb, Y.la, Y.lb, W.nblocks, d_E, ls)); ++launches; }
-      else {
-        // the roles of a class are separate kernels (slices of the bra function pairs of the same quartets): run them side by
-        // side on the role streams, forked from and joined to the launch's stream, so they share the pair data in L2 and one tail
-        const int nrs = std::min(nrole, TDG_ROLE_STREAMS);
-        if (nrs > 1) {
-          CK(cudaEventRecord(ctx->ev_rfork, ls));
-          for (int i = 1; i < nrs; ++i) CK(cudaStreamWaitEvent(ctx->rstream[i - 1], ctx->ev_rfork, 0));
-        }
-        for (int role = 0; role < nrole; ++role) {
-          tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb, role);
-          if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
-          const int ri = role % nrs;
-          fn(P, W.nblocks, ri == 0 ? ls : ctx->rstream[ri - 1]);
-          ++launches;
-        }
-        for (int i = 1; i < nrs; ++i) { CK(cudaEventRecord(ctx->ev_rjoin[i - 1], ctx->rstream[i - 1])); CK(cudaStreamWaitEvent(ls, ctx->ev_rjoin[i - 1], 0)); }
-      }
-      if (stats) { cudaEventRecord(e1, ls); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(W.cls); }
-    }
-    if (nstr > 1)
-      for (int i = 0; i < nstr - 1; ++i) { CK(cudaEventRecord(ctx->ev_join[i], ctx->side[i])); CK(cudaStreamWaitEvent(st, ctx->ev_join[i], 0)); }
   }
   CK(cudaGetLastError());
   if (d_E) {
@@ -751,23 +823,9 @@ extern "C" int tdg_fock(tdg_ctx* ctx, int nmat, const double* const* B, int matr
     CK(tdg_launch_pack(ps, n, ctx->d_bf2sh, ctx->d_shells, pk, st));
     CK(cudaMemsetAsync(G, 0, 4 * mbytes, st));
     aux_launches += 2;
-    for (size_t w = 0; w < nw; ++w) {
-      const Work& W = ctx->work[w];
-      const Bucket& X = ctx->buckets[W.b1]; const Bucket& Y = ctx->buckets[W.b2];
-      P.bra_hdr = X.d_hdr; P.bra_prim = X.d_prim; P.nbra = X.n; P.nppb = X.npp;
-      P.ket_hdr = Y.d_hdr; P.ket_prim = Y.d_prim; P.nket = Y.n; P.nppk = Y.npp;
-      P.cum = W.d_cum; P.ntiles = W.ntiles; P.same_bucket = (W.b1 == W.b2) ? 1 : 0;
-      P.counters = ctx->d_counters + 3 * (pass == 0 ? w : nw);
-      cudaEvent_t e0 = nullptr, e1 = nullptr;
-      if (stats) { e0 = pool.get(); e1 = pool.get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, st); }
-      const int nrole = tdg_num_roles(X.la, X.lb, Y.la, Y.lb);
-      for (int role = 0; role < nrole; ++role) {
-        tdg_launch_fn fn = tdg_get_launcher(X.la, X.lb, Y.la, Y.lb, role + TDG_FOCK_ROLE_BASE);
-        if (!fn) { ctx->err = "class kernel not built"; return TDG_EUNSUPPORTED; }
-        fn(P, W.nblocks, st);
-        ++launches;
-      }
-      if (stats) { cudaEventRecord(e1, st); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(W.cls); }
+    {
+      const int rc_l = launch_classes(ctx, P, TDG_FOCK_ROLE_BASE, nullptr, pass == 0, st, stats ? &pool : nullptr, evs, ev_cls, launches);
+      if (rc_l) return rc_l;
     }
     for (int s = s0; s < s1; ++s) {
       CK(tdg_launch_fock_finalize(G + (size_t)(s - s0) * n * n, n, slots[s].kind == 0 ? 1.0 : -1.0, fdev[slots[s].mat], st));

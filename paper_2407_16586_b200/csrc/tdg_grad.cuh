@@ -19,6 +19,7 @@
 #ifndef TDG_RU_LIM
 #define TDG_RU_LIM 120
 #endif
+#define TDG_MAX_ROLES_F 8
 #define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dd), f shells) use the block-per-quartet kernel (tdg_gradb.cuh)
 // target number of function quartets per role: 27 is the measured optimum (14: +30 %, 54: +15 % time on cfg 3), except
 // (dd|dp), which needs 54 to stay within TDG_MAX_ROLES (12 roles; 10x faster than the block-per-quartet kernel on cfg 3)
@@ -40,7 +41,9 @@ struct QC {
   static constexpr int RC = role_comps(LA, LB, LC, LD);
   static constexpr int ABN1 = RC / KDN >= NAB ? NAB : (RC / KDN > 0 ? RC / KDN : 1);
   static constexpr int NROLE1 = (NAB + ABN1 - 1) / ABN1;
-  static constexpr bool SMALL = NCOMP <= 27 || (!HASF && NROLE1 <= TDG_MAX_ROLES);   // fully unrolled code
+  // thread-per-quartet, fully unrolled code: up to 18 roles without f shells, up to 8 with (longer compiles; measured on cfg 2:
+  // the block-per-quartet kernel is 5-10x slower on the small f classes, which carry most of that config's quartets)
+  static constexpr bool SMALL = NCOMP <= 27 || NROLE1 <= (HASF ? TDG_MAX_ROLES_F : TDG_MAX_ROLES);
   static constexpr int NROLE = SMALL ? NROLE1 : 1;
   static constexpr int ABN = (NAB + NROLE - 1) / NROLE;
   static constexpr int UNR = SMALL ? 64 : 1;

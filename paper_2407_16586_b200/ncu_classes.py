@@ -41,7 +41,7 @@ METRICS = [
     "launch__registers_per_thread",
 ]
 HERE = os.path.dirname(os.path.abspath(__file__))
-_KERNEL = re.compile(r"tdg_grad(b?)_kernel<\(int\)(\d), \(int\)(\d), \(int\)(\d), \(int\)(\d)>")
+_KERNEL = re.compile(r"tdg_grad(b?)_kernel<(?:\(int\))?(\d), (?:\(int\))?(\d), (?:\(int\))?(\d), (?:\(int\))?(\d)[,>]")
 _UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12, "ns": 1.0, "us": 1e3, "usecond": 1e3, "ms": 1e6, "msecond": 1e6,
          "s": 1e9, "second": 1e9, "nsecond": 1.0}
 
