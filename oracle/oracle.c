@@ -30,7 +30,9 @@
  * K(T,T) vs explicit MO sum; energy vs numpy einsum over orc_eri_tensor; the density-weighted
  * screening rule (density_maxima, quartet_weight) vs the Cauchy-Schwarz inequality on every
  * density-weighted integral, the closed form for s shells, permutation/transpose invariance and
- * the c * n_dropped * tau error bound (tests/test_oracle_screening.py).
+ * the c * n_dropped * tau error bound (tests/test_oracle_screening.py).  One-electron terms (orc_onee_*, end of
+ * file): closed forms, finite differences of the pinned overlap, tight-charge limit of the pinned ERIs, mpmath
+ * derivatives of the s-s closed forms, finite differences of the energy (tests/test_oracle_onee.py).
  * Paper-printed values: none exist for this path ("parity unpinned" w.r.t. printed numbers).
  */
 #include <math.h>
@@ -955,4 +957,231 @@ int orc_num_threads(void) {
 #else
     return 1;
 #endif
+}
+
+/* ---------------------------------------------------------------- NEXT-4: one-electron terms of the gradient
+ * Terms 1-3 of PAPER.md:84 (eq 7):  g_A = sum_mn P_mn dH^core_mn/dA + sum_mn W_mn dS_mn/dA + dV_nuc/dA,
+ * H^core = T + V,  T_mn = <m| -1/2 Laplacian |n>,  V_mn = -sum_C Z_C <m| 1/|r - R_C| |n>,  V_nuc = sum_{C<D} Z_C Z_D / R_CD,
+ * with P and W held fixed (general matrices, not assumed symmetric).  The paper computes these on the CPU.
+ *
+ * Textbook McMurchie-Davidson, written out: per direction s_ij = E_0^{ij} sqrt(pi/p);
+ *   k_ij = -1/2 [ j(j-1) s_{i,j-2} - 2b(2j+1) s_{ij} + 4b^2 s_{i,j+2} ],   T = k_x s_y s_z + s_x k_y s_z + s_x s_y k_z;
+ *   V^C  = -Z_C (2 pi/p) sum_tuv E_t E_u E_v R_tuv(p, P - C),  R^n_000 = (-2p)^n F_n(p |P-C|^2).
+ * Derivatives, every centre explicitly (no translational-invariance shortcut): a function on A contributes
+ * d/dA_x = 2a [i+1] - i [i-1] (eq 39 with the nuclear-coordinate sign), same for B; the operator centre enters R through
+ * X = P_x - C_x, so d/dC_x R_tuv = -R_{t+1,u,v}.
+ * Pins (tests/test_oracle_onee.py): closed forms for s functions (S, T, V via erf), T = 1/2 sum_x d^2 S / dA_x dB_x by finite
+ * differences of the pinned overlap, V as the tight-charge limit of the pinned ERIs, hydrogen-like expectation values,
+ * gradient vs central finite differences of orc_onee_energy, sum over atoms = 0. */
+#define L1I (LMAX + 2)
+#define L1J (LMAX + 4)
+typedef double herm1_t[L1I][L1J][L1I + L1J + 1];
+
+static void hermite_E1(int imax, int jmax, double a, double b, double X, herm1_t E) {   /* same recurrences as hermite_E (O4) */
+    double p = a + b, mu = a * b / p;
+    for (int i = 0; i <= imax; ++i)
+        for (int j = 0; j <= jmax; ++j)
+            for (int t = 0; t <= L1I + L1J; ++t) E[i][j][t] = 0.0;
+    E[0][0][0] = exp(-mu * X * X);
+    for (int j = 0; j <= jmax; ++j) {
+        if (j > 0)
+            for (int t = 0; t <= j; ++t) {
+                double v = (a / p) * X * E[0][j - 1][t] + (t + 1) * E[0][j - 1][t + 1];
+                if (t > 0) v += E[0][j - 1][t - 1] / (2.0 * p);
+                E[0][j][t] = v;
+            }
+        for (int i = 1; i <= imax; ++i)
+            for (int t = 0; t <= i + j; ++t) {
+                double v = -(b / p) * X * E[i - 1][j][t] + (t + 1) * E[i - 1][j][t + 1];
+                if (t > 0) v += E[i - 1][j][t - 1] / (2.0 * p);
+                E[i][j][t] = v;
+            }
+    }
+}
+
+/* A 1-D factor of a (possibly differentiated) function: sum of at most two monomial powers with coefficients. */
+typedef struct { int n; int pw[2]; double co[2]; } lin1_t;
+static lin1_t lin_plain(int i) { lin1_t r; r.n = 1; r.pw[0] = i; r.co[0] = 1.0; r.pw[1] = 0; r.co[1] = 0.0; return r; }
+static lin1_t lin_deriv(int i, double zeta) {   /* d/d(centre): 2 zeta [i+1] - i [i-1] */
+    lin1_t r; r.n = 1; r.pw[0] = i + 1; r.co[0] = 2.0 * zeta; r.pw[1] = 0; r.co[1] = 0.0;
+    if (i > 0) { r.n = 2; r.pw[1] = i - 1; r.co[1] = -(double)i; }
+    return r;
+}
+static double s1d(herm1_t E, int i, int j, double p) { return (i < 0 || j < 0) ? 0.0 : E[i][j][0] * sqrt(PI / p); }
+static double k1d(herm1_t E, int i, int j, double b, double p) {
+    return -0.5 * (j * (j - 1) * s1d(E, i, j - 2, p) - 2.0 * b * (2 * j + 1) * s1d(E, i, j, p) + 4.0 * b * b * s1d(E, i, j + 2, p));
+}
+static double lin_s(herm1_t E, lin1_t u, lin1_t v, double p) {
+    double r = 0.0;
+    for (int x = 0; x < u.n; ++x) for (int y = 0; y < v.n; ++y) r += u.co[x] * v.co[y] * s1d(E, u.pw[x], v.pw[y], p);
+    return r;
+}
+static double lin_k(herm1_t E, lin1_t u, lin1_t v, double b, double p) {
+    double r = 0.0;
+    for (int x = 0; x < u.n; ++x) for (int y = 0; y < v.n; ++y) r += u.co[x] * v.co[y] * k1d(E, u.pw[x], v.pw[y], b, p);
+    return r;
+}
+static int lin_e(herm1_t E, lin1_t u, lin1_t v, double *out) {   /* Hermite vector of the product, entries t = 0..n-1 */
+    int n = 0;
+    for (int t = 0; t <= L1I + L1J; ++t) out[t] = 0.0;
+    for (int x = 0; x < u.n; ++x) for (int y = 0; y < v.n; ++y) {
+        int top = u.pw[x] + v.pw[y];
+        for (int t = 0; t <= top; ++t) out[t] += u.co[x] * v.co[y] * E[u.pw[x]][v.pw[y]][t];
+        if (top + 1 > n) n = top + 1;
+    }
+    return n;
+}
+
+/* One shell pair (si, sj): contracted, normalised S, T, V blocks [ni][nj] (any may be NULL), and, if acc != NULL, the pair's
+ * contribution sum_ab [ P_ab d(T+V)_ab + W_ab dS_ab ] to acc[3*natom] for all centres (A, B and every nucleus C). */
+static void onee_pair(const sys_t *s, const double *Zn, int si, int sj, double *Sb, double *Tb, double *Vb,
+                      const double *Pm, const double *Wm, double *acc, rtab_t R, double *rwork) {
+    const int32_t *sh = s->shells;
+    int la = sh[4 * si + 1], lb = sh[4 * sj + 1], na = ncart(la), nb = ncart(lb);
+    int atA = sh[4 * si], atB = sh[4 * sj];
+    const double *A = s->xyz + 3 * atA, *B = s->xyz + 3 * atB;
+    size_t n = (size_t)s->nbf;
+    int dv = acc ? 1 : 0;
+    if (Sb) memset(Sb, 0, sizeof(double) * (size_t)na * nb);
+    if (Tb) memset(Tb, 0, sizeof(double) * (size_t)na * nb);
+    if (Vb) memset(Vb, 0, sizeof(double) * (size_t)na * nb);
+    herm1_t E[3];
+    double G[MAXM];
+    for (int ka = 0; ka < sh[4 * si + 2]; ++ka)
+    for (int kb = 0; kb < sh[4 * sj + 2]; ++kb) {
+        double a = s->exps[sh[4 * si + 3] + ka], b = s->exps[sh[4 * sj + 3] + kb], p = a + b;
+        double Pc[3];
+        for (int x = 0; x < 3; ++x) { Pc[x] = (a * A[x] + b * B[x]) / p; hermite_E1(la + dv, lb + dv + 2, a, b, A[x] - B[x], E[x]); }
+        double cab = s->cn[sh[4 * si + 3] + ka] * s->cn[sh[4 * sj + 3] + kb];
+        for (int ia = 0; ia < na; ++ia)
+        for (int ib = 0; ib < nb; ++ib) {
+            int ax[3], bx[3];
+            cart_comp(la, ia, &ax[0], &ax[1], &ax[2]); cart_comp(lb, ib, &bx[0], &bx[1], &bx[2]);
+            double f = cab * comp_norm(ax[0], ax[1], ax[2]) * comp_norm(bx[0], bx[1], bx[2]);
+            double pw = Pm ? Pm[(size_t)(s->off[si] + ia) * n + s->off[sj] + ib] : 0.0;
+            double ww = Wm ? Wm[(size_t)(s->off[si] + ia) * n + s->off[sj] + ib] : 0.0;
+            /* variant 0: plain; 1..3: d/dA_x,y,z; 4..6: d/dB_x,y,z */
+            for (int var = 0; var < (dv ? 7 : 1); ++var) {
+                lin1_t u[3], v[3];
+                for (int x = 0; x < 3; ++x) {
+                    u[x] = (var >= 1 && var <= 3 && var - 1 == x) ? lin_deriv(ax[x], a) : lin_plain(ax[x]);
+                    v[x] = (var >= 4 && var - 4 == x) ? lin_deriv(bx[x], b) : lin_plain(bx[x]);
+                }
+                double sx = lin_s(E[0], u[0], v[0], p), sy = lin_s(E[1], u[1], v[1], p), sz = lin_s(E[2], u[2], v[2], p);
+                double kx = lin_k(E[0], u[0], v[0], b, p), ky = lin_k(E[1], u[1], v[1], b, p), kz = lin_k(E[2], u[2], v[2], b, p);
+                double Sv = f * sx * sy * sz;
+                double Tv = f * (kx * sy * sz + sx * ky * sz + sx * sy * kz);
+                double ex[L1I + L1J + 1], ey[L1I + L1J + 1], ez[L1I + L1J + 1];
+                int nx = lin_e(E[0], u[0], v[0], ex), ny = lin_e(E[1], u[1], v[1], ey), nz = lin_e(E[2], u[2], v[2], ez);
+                double Vv = 0.0;
+                for (int c = 0; c < s->natom; ++c) {
+                    if (Zn[c] == 0.0) continue;
+                    const double *Cc = s->xyz + 3 * c;
+                    double X = Pc[0] - Cc[0], Y = Pc[1] - Cc[1], Zd = Pc[2] - Cc[2];
+                    int N = la + lb + 2 * dv;
+                    orc_boys(N, p * (X * X + Y * Y + Zd * Zd), G);
+                    hermite_R(N, p, G, X, Y, Zd, R, rwork);
+                    double vc = 0.0, dC[3] = {0.0, 0.0, 0.0};
+                    for (int t = 0; t < nx; ++t) for (int uu = 0; uu < ny; ++uu) for (int w = 0; w < nz; ++w) {
+                        double e3 = ex[t] * ey[uu] * ez[w];
+                        vc += e3 * R[t][uu][w];
+                        if (var == 0 && dv) { dC[0] -= e3 * R[t + 1][uu][w]; dC[1] -= e3 * R[t][uu + 1][w]; dC[2] -= e3 * R[t][uu][w + 1]; }
+                    }
+                    double pref = -Zn[c] * 2.0 * PI / p * f;
+                    Vv += pref * vc;
+                    if (var == 0 && dv) for (int x = 0; x < 3; ++x) acc[3 * c + x] += pw * pref * dC[x];   /* operator centre */
+                }
+                if (var == 0) {
+                    if (Sb) Sb[ia * nb + ib] += Sv;
+                    if (Tb) Tb[ia * nb + ib] += Tv;
+                    if (Vb) Vb[ia * nb + ib] += Vv;
+                } else {
+                    int at = var <= 3 ? atA : atB, x = (var - 1) % 3;
+                    acc[3 * at + x] += pw * (Tv + Vv) + ww * Sv;
+                }
+            }
+        }
+    }
+}
+
+int orc_onee_matrices(SYS_ARGS, const double *Z, double *S, double *T, double *V) {
+    sys_t s; int rc = sys_init(&s, SYS_PASS); if (rc) return rc;
+    size_t n = (size_t)s.nbf;
+    double *rwork = (double *)malloc(sizeof(double) * (size_t)(NTOT + 1) * (NTOT + 1) * (NTOT + 1) * (NTOT + 1));
+    rtab_t *R = (rtab_t *)malloc(sizeof(rtab_t));
+    double Sb[NCMAX * NCMAX], Tb[NCMAX * NCMAX], Vb[NCMAX * NCMAX];
+    for (int i = 0; i < nshell; ++i) for (int j = 0; j < nshell; ++j) {
+        onee_pair(&s, Z, i, j, Sb, Tb, Vb, NULL, NULL, NULL, *R, rwork);
+        int ni = s.off[i + 1] - s.off[i], nj = s.off[j + 1] - s.off[j];
+        for (int a = 0; a < ni; ++a) for (int b = 0; b < nj; ++b) {
+            size_t idx = (size_t)(s.off[i] + a) * n + s.off[j] + b;
+            S[idx] = Sb[a * nj + b]; T[idx] = Tb[a * nj + b]; V[idx] = Vb[a * nj + b];
+        }
+    }
+    free(R); free(rwork); sys_free(&s);
+    return 0;
+}
+
+static double vnuc(const sys_t *s, const double *Z, double *grad) {
+    double e = 0.0;
+    for (int c = 0; c < s->natom; ++c) for (int d = 0; d < c; ++d) {
+        double r[3], r2 = 0.0;
+        for (int x = 0; x < 3; ++x) { r[x] = s->xyz[3 * c + x] - s->xyz[3 * d + x]; r2 += r[x] * r[x]; }
+        double rr = sqrt(r2);
+        e += Z[c] * Z[d] / rr;
+        if (grad) for (int x = 0; x < 3; ++x) { double gx = -Z[c] * Z[d] * r[x] / (r2 * rr); grad[3 * c + x] += gx; grad[3 * d + x] -= gx; }
+    }
+    return e;
+}
+
+/* E_1e = sum_mn P_mn (T + V)_mn + sum_mn W_mn S_mn + V_nuc. */
+int orc_onee_energy(SYS_ARGS, const double *Z, const double *P, const double *W, double *E) {
+    sys_t s; int rc = sys_init(&s, SYS_PASS); if (rc) return rc;
+    size_t n = (size_t)s.nbf;
+    double *rwork = (double *)malloc(sizeof(double) * (size_t)(NTOT + 1) * (NTOT + 1) * (NTOT + 1) * (NTOT + 1));
+    rtab_t *R = (rtab_t *)malloc(sizeof(rtab_t));
+    double Sb[NCMAX * NCMAX], Tb[NCMAX * NCMAX], Vb[NCMAX * NCMAX];
+    double e = 0.0;
+    for (int i = 0; i < nshell; ++i) for (int j = 0; j < nshell; ++j) {
+        onee_pair(&s, Z, i, j, Sb, Tb, Vb, NULL, NULL, NULL, *R, rwork);
+        int ni = s.off[i + 1] - s.off[i], nj = s.off[j + 1] - s.off[j];
+        for (int a = 0; a < ni; ++a) for (int b = 0; b < nj; ++b) {
+            size_t idx = (size_t)(s.off[i] + a) * n + s.off[j] + b;
+            e += P[idx] * (Tb[a * nj + b] + Vb[a * nj + b]) + W[idx] * Sb[a * nj + b];
+        }
+    }
+    *E = e + vnuc(&s, Z, NULL);
+    free(R); free(rwork); sys_free(&s);
+    return 0;
+}
+
+/* grad[natom][3] = dE_1e/dR with P, W fixed: terms 1-3 of eq 7.  All nshell^2 ordered shell pairs. */
+int orc_onee_gradient(SYS_ARGS, const double *Z, const double *P, const double *W, double *grad) {
+    sys_t s; int rc = sys_init(&s, SYS_PASS); if (rc) return rc;
+    size_t ng = 3 * (size_t)natom;
+    memset(grad, 0, sizeof(double) * ng);
+    int nthr = 1;
+#ifdef _OPENMP
+    nthr = omp_get_max_threads();
+#endif
+    double *acc = (double *)calloc(ng * (size_t)nthr, sizeof(double));
+    if (!acc) { sys_free(&s); return -1; }
+#pragma omp parallel
+    {
+        int th = 0;
+#ifdef _OPENMP
+        th = omp_get_thread_num();
+#endif
+        double *rwork = (double *)malloc(sizeof(double) * (size_t)(NTOT + 1) * (NTOT + 1) * (NTOT + 1) * (NTOT + 1));
+        rtab_t *R = (rtab_t *)malloc(sizeof(rtab_t));
+#pragma omp for schedule(dynamic, 1)
+        for (int i = 0; i < nshell; ++i)
+            for (int j = 0; j < nshell; ++j)
+                onee_pair(&s, Z, i, j, NULL, NULL, NULL, P, W, acc + ng * (size_t)th, *R, rwork);
+        free(R); free(rwork);
+    }
+    for (int th = 0; th < nthr; ++th) for (size_t t = 0; t < ng; ++t) grad[t] += acc[ng * (size_t)th + t];
+    vnuc(&s, Z, grad);
+    free(acc); sys_free(&s);
+    return 0;
 }

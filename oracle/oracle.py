@@ -227,6 +227,48 @@ def sph_transform(sysm, flags) -> np.ndarray:
     return Cm
 
 
+def _onee_in(sysm, Z, P=None, W=None):
+    Z = np.ascontiguousarray(Z, dtype=np.float64)
+    assert Z.shape == (sysm.natom,)
+    n = sysm.nbf
+    P = None if P is None else np.ascontiguousarray(P, dtype=np.float64)
+    W = None if W is None else np.ascontiguousarray(W, dtype=np.float64)
+    for M in (P, W):
+        assert M is None or M.shape == (n, n)
+    return Z, P, W
+
+
+def onee_matrices(sysm, Z):
+    """S, T (kinetic), V (nuclear attraction, charges Z[natom]) over the normalised Cartesian functions (NEXT-4)."""
+    args, keep = _sys_args(sysm)
+    Z, _, _ = _onee_in(sysm, Z)
+    n = sysm.nbf
+    S, T, V = np.zeros((n, n)), np.zeros((n, n)), np.zeros((n, n))
+    rc = lib().orc_onee_matrices(*args, Z.ctypes.data_as(C.c_void_p), *[x.ctypes.data_as(C.c_void_p) for x in (S, T, V)])
+    assert rc == 0, rc
+    return S, T, V
+
+
+def onee_energy(sysm, Z, P, W) -> float:
+    """sum P (T + V) + sum W S + V_nuc."""
+    args, keep = _sys_args(sysm)
+    Z, P, W = _onee_in(sysm, Z, P, W)
+    e = np.zeros(1)
+    rc = lib().orc_onee_energy(*args, *[x.ctypes.data_as(C.c_void_p) for x in (Z, P, W, e)])
+    assert rc == 0, rc
+    return float(e[0])
+
+
+def onee_gradient(sysm, Z, P, W) -> np.ndarray:
+    """Terms 1-3 of eq 7: sum P dH^core + sum W dS + dV_nuc, [natom, 3]."""
+    args, keep = _sys_args(sysm)
+    Z, P, W = _onee_in(sysm, Z, P, W)
+    g = np.zeros(3 * sysm.natom)
+    rc = lib().orc_onee_gradient(*args, *[x.ctypes.data_as(C.c_void_p) for x in (Z, P, W, g)])
+    assert rc == 0, rc
+    return g.reshape(-1, 3)
+
+
 def sample_keep(i, j, k, l, mod, seed) -> bool:
     return bool(lib().orc_sample_keep(C.c_int(i), C.c_int(j), C.c_int(k), C.c_int(l), C.c_uint32(mod), C.c_uint32(seed)))
 
