@@ -137,6 +137,20 @@ int tdg_energy(tdg_ctx* ctx, int npair, const double* const* A, const double* co
                const double* wJ, const double* wK, double cJ, double cK, double cLR, double omega,
                void* stream, double* E_host);
 
+/* One-electron terms of the gradient (terms 1-3 of eq 7; evaluated on the CPU in the paper,
+ * PAPER.md:404):
+ *
+ *   grad[E][x] = sum_mn P_mn d(T + V)_mn/dR_{E,x} + sum_mn W_mn dS_mn/dR_{E,x} + dV_nuc/dR_{E,x}
+ *
+ * S overlap, T = <m|-1/2 Laplacian|n>, V_mn = -sum_C Z_C <m|1/|r - R_C||n>, V_nuc = sum_{C<D} Z_C Z_D / R_CD; P (the density of
+ * eq 8) and W (the energy-weighted density of eq 7) are held fixed, general nbf x nbf row-major matrices in the input basis of
+ * tdg_nbf (all device pointers if matrices_on_device != 0, else host; either may be NULL = zero).  Z[natom]: nuclear charges, HOST.
+ * Runs over the shell pairs kept by tdg_plan (pairs with Q_ij Q_max < tau are dropped here too; tau = 0 keeps all).
+ * grad: [natom][3], device pointer if grad_on_device != 0 else host; overwritten.  The call synchronises the stream (Z is a host
+ * array).  ms (may be NULL): device time of the call.  Not concurrent with other calls on the same context. */
+int tdg_onee_gradient(tdg_ctx* ctx, const double* Z, const double* P, const double* W, int matrices_on_device, void* stream,
+                      double* grad, int grad_on_device, float* ms);
+
 /* Fock-type (J/K) build, integral-direct with the same plan, screening and kernels' machinery as tdg_gradient (SURVEY.md 8(f)
  * NEXT-1).  For each of the nmat input matrices B_k (nbf x nbf row-major, general; all device or all host pointers):
  *

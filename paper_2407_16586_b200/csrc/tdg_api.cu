@@ -873,6 +873,37 @@ extern "C" int tdg_fock(tdg_ctx* ctx, int nmat, const double* const* B, int matr
   return TDG_OK;
 }
 
+// ---- NEXT-4: one-electron terms of the gradient (eq 7 terms 1-3; kernels in tdg_onee.cu) ----
+extern "C" int tdg_onee_gradient(tdg_ctx* ctx, const double* Z, const double* Pm, const double* Wm, int matrices_on_device, void* stream,
+                                 double* grad, int grad_on_device, float* ms) {
+  if (!ctx || !Z || !grad) return TDG_EINVAL;
+  if (!ctx->planned) return TDG_ENOTPLANNED;
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  std::fill(ctx->scratch_used.begin(), ctx->scratch_used.end(), false);
+  EventPool pool;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  if (ms) { ev0 = pool.get(); ev1 = pool.get(); if (!ev0 || !ev1) return TDG_ECUDA; cudaEventRecord(ev0, st); }
+  const double *dP = nullptr, *dW = nullptr;
+  if (Pm) { const int rc = to_device_cart(ctx, Pm, matrices_on_device, st, &dP); if (rc) return rc; }
+  if (Wm) { const int rc = to_device_cart(ctx, Wm, matrices_on_device, st, &dW); if (rc) return rc; }
+  double* dZ = (double*)scratch_get(ctx, sizeof(double) * ctx->natom + 16);
+  if (!dZ) { ctx->err = "device allocation of the nuclear charges failed"; return TDG_ENOMEM; }
+  CK(cudaMemcpyAsync(dZ, Z, sizeof(double) * ctx->natom, cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(ctx->d_grad, 0, sizeof(double) * 3 * ctx->natom, st));
+  if (dP || dW)
+    for (const Bucket& X : ctx->buckets)
+      CK(tdg_launch_onee(X.d_hdr, X.d_prim, X.n, X.npp, X.la, X.lb, ctx->d_xyz, dZ, ctx->natom, dP, dW, ctx->nbf, ctx->d_grad, ctx->d_rys, st));
+  CK(tdg_launch_vnuc_grad(ctx->d_xyz, dZ, ctx->natom, ctx->d_grad, st));
+  const size_t gb = sizeof(double) * 3 * ctx->natom;
+  if (grad_on_device) CK(cudaMemcpyAsync(grad, ctx->d_grad, gb, cudaMemcpyDeviceToDevice, st));
+  else CK(cudaMemcpyAsync(grad, ctx->d_grad, gb, cudaMemcpyDeviceToHost, st));
+  if (ms) cudaEventRecord(ev1, st);
+  CK(cudaStreamSynchronize(st));   // Z (and host matrices) are the caller's host arrays: their uploads finish before the call returns
+  if (ms) cudaEventElapsedTime(ms, ev0, ev1);
+  return TDG_OK;
+}
+
 extern "C" int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out) {
   if (!ctx || !T || !rho || !out || n < 1 || n > 7 || count <= 0) return TDG_EINVAL;
   cudaSetDevice(ctx->device);

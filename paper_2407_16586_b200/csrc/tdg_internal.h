@@ -36,3 +36,9 @@ cudaError_t tdg_launch_fock_finalize(const double* G, int n, double sign, double
 // gradient kernels; *E (device) is accumulated with FP64 atomics.
 struct KParams;
 cudaError_t tdg_launch_energy(const KParams& P, int la, int lb, int lc, int ld, int nblocks, double* E, cudaStream_t s);
+
+// One-electron gradient terms (tdg_onee.cu; NEXT-4): one launch per pair bucket; grad is accumulated with FP64 atomics.
+struct PairHdr;
+cudaError_t tdg_launch_onee(const PairHdr* hdr, const double* prim, int npair, int npp, int la, int lb, const double* xyz, const double* Z,
+                            int natom, const double* Pm, const double* Wm, int nbf, double* grad, const double* rys_tab, cudaStream_t s);
+cudaError_t tdg_launch_vnuc_grad(const double* xyz, const double* Z, int natom, double* grad, cudaStream_t s);

@@ -17,7 +17,7 @@ NCLASS = 55
 _lib = None
 
 SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_spherical", "tdg_set_shard", "tdg_set_streams", "tdg_plan", "tdg_schwarz", "tdg_gradient",
-           "tdg_energy", "tdg_fock", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
+           "tdg_energy", "tdg_fock", "tdg_onee_gradient", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
 
 
 class TdgError(RuntimeError):
@@ -256,6 +256,21 @@ class Context:
                             C.c_double(omega), C.c_void_p(stream if stream else 0), PF, C.c_int(f_dev), C.byref(st) if st is not None else None)
         self._check(rc, "tdg_fock")
         return F, (st.asdict() if st is not None else None)
+
+    def onee_gradient(self, Z, P, W, stream=None, out=None):
+        """One-electron terms sum P d(T+V) + sum W dS + dV_nuc (include/tdgrad.h: tdg_onee_gradient).  Z: nuclear charges [natom];
+        P, W: numpy arrays (host) or CUDA torch tensors (or None = zero).  Returns (gradient [natom, 3] as numpy array or ``out``, ms)."""
+        Z = np.ascontiguousarray(Z, dtype=np.float64)
+        mats = [m for m in (P, W) if m is not None]
+        on_dev = 0 if (not mats or isinstance(mats[0], np.ndarray)) else 1
+        keep = [None if m is None else (np.ascontiguousarray(m, dtype=np.float64) if not on_dev else m) for m in (P, W)]
+        g = np.zeros((self.natom, 3)) if out is None else out
+        ms = C.c_float()
+        rc = lib().tdg_onee_gradient(self._h, C.c_void_p(Z.ctypes.data), *[C.c_void_p(_ptr(m)) if m is not None else None for m in keep],
+                                     C.c_int(on_dev), C.c_void_p(stream if stream else 0), C.c_void_p(_ptr(g)), C.c_int(0 if out is None else 1),
+                                     C.byref(ms))
+        self._check(rc, "tdg_onee_gradient")
+        return g, ms.value
 
     def rys(self, n, T, rho=None, omega=0.0) -> np.ndarray:
         T = np.ascontiguousarray(T, dtype=np.float64)
