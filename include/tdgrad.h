@@ -172,6 +172,20 @@ int tdg_fock(tdg_ctx* ctx, int nmat, const double* const* B, int matrices_on_dev
  * s^2 = omega^2/(omega^2+rho)).  Runs on the device.  1 <= n <= 7. */
 int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, double* out);
 
+/* Allocation-free variant of tdg_rys for callers that may not call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid allocation).  Same arithmetic and the same arguments and result layout as tdg_rys (n = 1..7 roots;
+ * T, rho, out are HOST arrays of count and count*2n doubles; per evaluation x_0..x_{n-1}, w_0..w_{n-1}), but every byte of device
+ * workspace is a fixed file-scope device array of the library (csrc/tdg_noalloc.cu): 2 MiB + 256 B, held by every GPU that loads
+ * the library until the process exits.  The call makes NO cudaMalloc / cudaFree / allocating library call (tdg_create, which
+ * uploads the Rys tables, has to have happened before).  Limit: 1 <= count <= TDG_RYS_STATIC_MAX, larger counts are rejected with
+ * TDG_EINVAL and a text in tdg_last_error (split the batch).  Arguments with T < 0, rho <= 0, NaN or infinite are rejected with
+ * TDG_EINVAL as well (out is then unspecified).  stream: cudaStream_t as void* or NULL; the call synchronises it.
+ * ALL calls on one GPU share the array, which keeps the last call's contents (each call overwrites what it reads and clears its
+ * error counter): calls that overlap on the GPU - other streams, other host threads, other contexts on the same device - RACE;
+ * serialise them. */
+#define TDG_RYS_STATIC_MAX 16384
+int tdg_rys_static(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, void* stream, double* out);
+
 /* FP64 FMA throughput microbenchmark on this device (the roofline denominator; step 8d): runs chains of
  * dependent DFMAs on all SMs for about `ms` milliseconds; writes achieved TFLOP/s (2 flop per FMA). */
 int tdg_fp64_peak(tdg_ctx* ctx, double ms, double* tflops);

@@ -39,6 +39,7 @@ DEPS = {   # headers each source includes
     "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "rys_meta.inc"],
     "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
     "tdg_onee.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc"],
+    "tdg_noalloc.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc"],
     "tdg_api.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_internal.h", "tdg_classes.inc", "rys_meta.inc", "../../include/tdgrad.h"],
 }
 
@@ -68,7 +69,7 @@ def _same_flags(obj, extra) -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     jobs = [("tdg_api.cu", os.path.join(OBJ, "tdg_api.o"), []), ("tdg_aux.cu", os.path.join(OBJ, "tdg_aux.o"), []),
-            ("tdg_onee.cu", os.path.join(OBJ, "tdg_onee.o"), [])]
+            ("tdg_onee.cu", os.path.join(OBJ, "tdg_onee.o"), []), ("tdg_noalloc.cu", os.path.join(OBJ, "tdg_noalloc.o"), [])]
     for la, lb, lc, ld in QUARTET_CLASSES:
         for role in range(num_roles(la, lb, lc, ld)):   # one translation unit per (class, role): they compile in parallel
             jobs.append(("tdg_class.cu", os.path.join(OBJ, "tdg_class_%d%d%d%d_r%d.o" % (la, lb, lc, ld, role)),

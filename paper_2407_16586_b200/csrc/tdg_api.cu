@@ -948,6 +948,21 @@ extern "C" int tdg_rys(tdg_ctx* ctx, int n, int count, const double* T, const do
   return TDG_OK;
 }
 
+// Allocation-free variant of tdg_rys (workspace: the file-scope device array of tdg_noalloc.cu; no cudaMalloc / cudaFree here).
+extern "C" int tdg_rys_static(tdg_ctx* ctx, int n, int count, const double* T, const double* rho, double omega, void* stream, double* out) {
+  if (!ctx || !T || !rho || !out || n < 1 || n > 7 || count <= 0) return TDG_EINVAL;
+  if (count > tdg_rys_static_max()) {
+    ctx->err = "tdg_rys_static: count " + std::to_string(count) + " exceeds the fixed workspace (TDG_RYS_STATIC_MAX = " +
+               std::to_string(tdg_rys_static_max()) + " evaluations per call); split the batch or use tdg_rys";
+    return TDG_EINVAL;
+  }
+  cudaSetDevice(ctx->device);
+  unsigned long long nbad = 0;
+  CK(tdg_run_rys_static(ctx->device, n, count, T, rho, omega, ctx->d_rys, out, &nbad, (cudaStream_t)stream));
+  if (nbad) { ctx->err = "tdg_rys_static: " + std::to_string(nbad) + " argument(s) with T < 0, rho <= 0, NaN or infinity"; return TDG_EINVAL; }
+  return TDG_OK;
+}
+
 extern "C" int tdg_fp64_peak(tdg_ctx* ctx, double ms, double* tflops) {
   if (!ctx || !tflops) return TDG_EINVAL;
   cudaSetDevice(ctx->device);

@@ -42,3 +42,9 @@ struct PairHdr;
 cudaError_t tdg_launch_onee(const PairHdr* hdr, const double* prim, int npair, int npp, int la, int lb, const double* xyz, const double* Z,
                             int natom, const double* Pm, const double* Wm, int nbf, double* grad, const double* rys_tab, cudaStream_t s);
 cudaError_t tdg_launch_vnuc_grad(const double* xyz, const double* Z, int natom, double* grad, cudaStream_t s);
+
+// Allocation-free Rys evaluation (tdg_noalloc.cu): all device workspace in a file-scope __device__ array; count <= TDG_RYS_STATIC_MAX.
+#define TDG_RYS_STATIC_MAX 16384
+int tdg_rys_static_max(void);
+cudaError_t tdg_run_rys_static(int device, int n, int count, const double* T, const double* rho, double omega, const double* tab, double* out,
+                               unsigned long long* nbad, cudaStream_t s);

@@ -17,7 +17,10 @@ NCLASS = 55
 _lib = None
 
 SYMBOLS = ["tdg_create", "tdg_destroy", "tdg_set_system", "tdg_nbf", "tdg_set_spherical", "tdg_set_shard", "tdg_set_streams", "tdg_plan", "tdg_schwarz", "tdg_gradient",
-           "tdg_energy", "tdg_fock", "tdg_onee_gradient", "tdg_rys", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
+           "tdg_energy", "tdg_fock", "tdg_onee_gradient", "tdg_rys", "tdg_rys_static", "tdg_fp64_peak", "tdg_strerror", "tdg_last_error"]
+
+
+RYS_STATIC_MAX = 16384   # TDG_RYS_STATIC_MAX of include/tdgrad.h
 
 
 class TdgError(RuntimeError):
@@ -279,6 +282,16 @@ class Context:
         rc = lib().tdg_rys(self._h, C.c_int(n), C.c_int(T.shape[0]), C.c_void_p(T.ctypes.data), C.c_void_p(rho.ctypes.data),
                            C.c_double(omega), C.c_void_p(out.ctypes.data))
         self._check(rc, "tdg_rys")
+        return out
+
+    def rys_static(self, n, T, rho=None, omega=0.0, stream=None) -> np.ndarray:
+        """tdg_rys without any allocation on the device (include/tdgrad.h: tdg_rys_static; at most RYS_STATIC_MAX evaluations per call)."""
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        rho = np.ones_like(T) if rho is None else np.ascontiguousarray(rho, dtype=np.float64)
+        out = np.zeros((T.shape[0], 2 * n))
+        rc = lib().tdg_rys_static(self._h, C.c_int(n), C.c_int(T.shape[0]), C.c_void_p(T.ctypes.data), C.c_void_p(rho.ctypes.data),
+                                  C.c_double(omega), C.c_void_p(stream if stream else 0), C.c_void_p(out.ctypes.data))
+        self._check(rc, "tdg_rys_static")
         return out
 
     def fp64_peak(self, ms=300.0) -> float:
