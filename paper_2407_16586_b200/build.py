@@ -36,7 +36,7 @@ def num_roles(la: int, lb: int, lc: int, ld: int) -> int:
     small = nab * kdn <= 27 or nrole1 <= (8 if 3 in (la, lb, lc, ld) else 18)
     return nrole1 if small else 1
 DEPS = {   # headers each source includes
-    "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "rys_meta.inc"],
+    "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "tdg_fock.cuh", "rys_meta.inc"],
     "tdg_aux.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc", "rys_tables.inc", "boys_tables.inc"],
     "tdg_onee.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc"],
     "tdg_noalloc.cu": ["tdg_common.cuh", "tdg_internal.h", "rys_meta.inc"],

@@ -554,6 +554,12 @@ static int launch_classes(tdg_ctx* ctx, KParams& P, int role_base, double* d_E, 
                           std::vector<cudaEvent_t>& evs, std::vector<int>& ev_cls, int& launches) {
   const size_t nw = ctx->work.size();
   const int nstr = d_E ? 1 : ctx->nstreams;
+  // With per-class timing (stats requested) the side streams join the caller's stream after every class, so that the events time
+  // exactly that class; without it they fork once before the first class and join once after the last, and the tail of one class
+  // overlaps the start of the next (the tails are the part of a call that does not shrink when the work is sharded over ranks).
+  // Measured on cfg 3 (profiles/r02_shard_balance_cfg3.md): free-running is 13 % faster on a 1/8 shard, 5 % on a 1/4 shard, and
+  // 1.7 % SLOWER on the whole problem (kernels of different classes then share the SMs for longer), so it is used for shards only.
+  const bool join_per_class = pool != nullptr || nstr == 1 || ctx->shard_n == 1;
   std::vector<size_t> order(nw);
   for (size_t w = 0; w < nw; ++w) order[w] = w;
   std::stable_sort(order.begin(), order.end(), [&](size_t x, size_t y) { return ctx->work[x].cls < ctx->work[y].cls; });
@@ -562,11 +568,11 @@ static int launch_classes(tdg_ctx* ctx, KParams& P, int role_base, double* d_E, 
     while (g1 < nw && ctx->work[order[g1]].cls == ctx->work[order[g0]].cls) ++g1;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (pool) { e0 = pool->get(); e1 = pool->get(); if (!e0 || !e1) return TDG_ECUDA; cudaEventRecord(e0, st); }
-    if (nstr > 1) {
+    if (nstr > 1 && (join_per_class || g0 == 0)) {
       CK(cudaEventRecord(ctx->ev_fork, st));
       for (int i = 0; i < nstr - 1; ++i) CK(cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
     }
-    int unit = 0;
+    int unit = join_per_class ? 0 : (int)g0;   // free-running: keep dealing round-robin across the class boundary
     for (size_t gw = g0; gw < g1; ++gw) {
       const size_t w = order[gw];
       const Work& W = ctx->work[w];
@@ -585,7 +591,7 @@ static int launch_classes(tdg_ctx* ctx, KParams& P, int role_base, double* d_E, 
         ++launches;
       }
     }
-    if (nstr > 1)
+    if (nstr > 1 && (join_per_class || g1 == nw))
       for (int i = 0; i < nstr - 1; ++i) { CK(cudaEventRecord(ctx->ev_join[i], ctx->side[i])); CK(cudaStreamWaitEvent(st, ctx->ev_join[i], 0)); }
     if (pool) { cudaEventRecord(e1, st); evs.push_back(e0); evs.push_back(e1); ev_cls.push_back(ctx->work[order[g0]].cls); }
     g0 = g1;

@@ -12,7 +12,7 @@ static void launch(const KParams& P, int nblocks, cudaStream_t s) {
   typedef QC<TDG_LA, TDG_LB, TDG_LC, TDG_LD> C;
   // the shared-memory attribute is per device and the call is cheap: set it on every launch (contexts may live on several devices)
   if constexpr (C::SMALL) {   // one thread per quartet, registers only (tdg_grad.cuh)
-    constexpr int smem = (C::RYS_SH_DOUBLES + TDG_ACC_DOUBLES) * (int)sizeof(double);
+    constexpr int smem = (C::RYS_SH_DOUBLES + C::IJ_SH_DOUBLES + TDG_ACC_DOUBLES) * (int)sizeof(double);
     cudaFuncSetAttribute(tdg_grad_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, TDG_ROLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     tdg_grad_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, TDG_ROLE><<<nblocks, TDG_WARPS * TDG_WARP, smem, s>>>(P);
   } else {                    // one block per quartet, 2-D integrals in shared memory (tdg_gradb.cuh)
@@ -28,7 +28,7 @@ static void launch_fock(const KParams& P, int nblocks, cudaStream_t s) {
   typedef QC<TDG_LA, TDG_LB, TDG_LC, TDG_LD> C;
   if constexpr (C::SMALL) {
     constexpr int nr = (TDG_LA + TDG_LB + TDG_LC + TDG_LD) / 2 + 1;
-    constexpr int smem = nr <= 4 ? rys_part_doubles(nr) * (int)sizeof(double) : 0;
+    constexpr int smem = nr <= 4 ? rys_sh_doubles(nr) * (int)sizeof(double) : 0;
     cudaFuncSetAttribute(tdg_fock_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, TDG_ROLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     tdg_fock_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, TDG_ROLE><<<nblocks, TDG_WARPS * TDG_WARP, smem, s>>>(P);
   } else {

@@ -107,7 +107,16 @@ __host__ __device__ inline bool tdg_sample_keep(int i, int j, int k, int l, uint
 // `tabN` points at the table of this N (global: tab + rys_off(N); or a copy of it staged in shared memory, where the
 // lanes' different intervals cost bank conflicts instead of one L1 wavefront per lane).
 #define RYS_TABLE_DOUBLES(N) (rys_tmax(N) * (RYS_DEG + 1) * 2 * (N))
-template <int N>
+// Shared-memory layout of a staged table (SH = true; rys_sh_index maps the global layout to it).  Lanes evaluate different T, so
+// they read different rows; in the global layout the rows of the lanes start at a few bank offsets only (Boys rows: 64 bytes, two
+// offsets; polynomial intervals: 672 bytes for n = 3, four offsets; 896 bytes for n = 4, ONE offset) and a 128-bit load of a warp
+// costs 8-32 wavefronts instead of 4.  Staged layout: n <= 2: the four 16-byte chunks of Boys row r are stored at chunk ^ ((r >> 1) & 3);
+// n >= 3: every interval is padded by 16 bytes.  Either way consecutive rows cycle through all eight 16-byte bank groups.
+#ifndef TDG_RYS_SH_LAYOUT
+#define TDG_RYS_SH_LAYOUT 1
+#endif
+#define RYS_SH_PAD (TDG_RYS_SH_LAYOUT ? 2 : 0)   // doubles of padding per polynomial interval
+template <int N, bool SH = false>
 __device__ __forceinline__ void rys_roots_tab(const double* __restrict__ tabN, double T, double* __restrict__ x, double* __restrict__ w) {
   if (T >= (double)rys_tmax(N)) {
     double rT = 1.0 / T, rs = sqrt(rT);
@@ -117,7 +126,7 @@ __device__ __forceinline__ void rys_roots_tab(const double* __restrict__ tabN, d
   }
   int i = (int)T;                       // RYS_H == 1
   double u = (T - ((double)i + 0.5)) * 2.0;
-  const double2* c = reinterpret_cast<const double2*>(tabN + i * ((RYS_DEG + 1) * 2 * N));   // rows of 2N doubles: 16-byte aligned
+  const double2* c = reinterpret_cast<const double2*>(tabN + i * ((RYS_DEG + 1) * 2 * N + (SH ? RYS_SH_PAD : 0)));   // rows of 2N doubles: 16-byte aligned
   double2 v[N];
 #pragma unroll
   for (int f = 0; f < N; ++f) v[f] = c[f];
@@ -138,7 +147,7 @@ __device__ __forceinline__ void rys_roots_tab(const double* __restrict__ tabN, d
 // and the roots of the monic orthogonal quadratic of the 2x2 Hankel system for n = 2).  boys_tables.inc layout.
 #define BOYS_PER_UNIT 8
 #define BOYS_K 8
-template <int N>
+template <int N, bool SH = false>
 __device__ __forceinline__ void rys_roots_boys(const double* __restrict__ tabN, double T, double* __restrict__ x, double* __restrict__ w) {
   static_assert(N == 1 || N == 2, "closed form only for n <= 2");
   if (T >= (double)rys_tmax(N)) {
@@ -150,7 +159,8 @@ __device__ __forceinline__ void rys_roots_boys(const double* __restrict__ tabN, 
   const int i = (int)(T * BOYS_PER_UNIT);
   const double d = T - ((double)i + 0.5) * (1.0 / BOYS_PER_UNIT);
   const double2* c = reinterpret_cast<const double2*>(tabN + i * BOYS_K);
-  const double2 c01 = c[0], c23 = c[1], c45 = c[2], c67 = c[3];
+  const int sw = (SH && TDG_RYS_SH_LAYOUT) ? ((i >> 1) & 3) : 0;
+  const double2 c01 = c[sw], c23 = c[1 ^ sw], c45 = c[2 ^ sw], c67 = c[3 ^ sw];
   double F = fma(c67.y, d, c67.x);
   F = fma(F, d, c45.y); F = fma(F, d, c45.x); F = fma(F, d, c23.y); F = fma(F, d, c23.x); F = fma(F, d, c01.y); F = fma(F, d, c01.x);
   const double e = exp(-T), T2 = 2.0 * T;
@@ -174,10 +184,20 @@ __device__ __forceinline__ void rys_roots_boys(const double* __restrict__ tabN, 
 __host__ __device__ constexpr int rys_part_off(int n) { return n <= 2 ? rys_off(RYS_NMAX + 1) + (n == 2 ? rys_tmax(1) * BOYS_PER_UNIT * BOYS_K : 0) : rys_off(n); }
 __host__ __device__ constexpr int rys_part_doubles(int n) { return n <= 2 ? rys_tmax(n) * BOYS_PER_UNIT * BOYS_K : RYS_TABLE_DOUBLES(n); }
 // `part` points at rys_part_off(N) of the device table (or at a shared-memory copy of that part)
-template <int N>
+template <int N, bool SH = false>
 __device__ __forceinline__ void rys_eval(const double* __restrict__ part, double T, double* __restrict__ x, double* __restrict__ w) {
-  if constexpr (N <= 2) rys_roots_boys<N>(part, T, x, w);
-  else rys_roots_tab<N>(part, T, x, w);
+  if constexpr (N <= 2) rys_roots_boys<N, SH>(part, T, x, w);
+  else rys_roots_tab<N, SH>(part, T, x, w);
+}
+// Staged (shared-memory) size of the part, and position of double2 element i of the global part in the staged layout.
+__host__ __device__ constexpr int rys_sh_doubles(int n) { return n <= 2 ? rys_part_doubles(n) : rys_part_doubles(n) + rys_tmax(n) * RYS_SH_PAD; }
+template <int N>
+__device__ __forceinline__ int rys_sh_index(int i) {
+  if (!TDG_RYS_SH_LAYOUT) return i;
+  if (N <= 2) { const int row = i >> 2, chunk = i & 3; return (row << 2) | (chunk ^ ((row >> 1) & 3)); }
+  constexpr int per = (RYS_DEG + 1) * N;     // double2 elements per interval
+  const int iv = i / per;
+  return i + iv * (RYS_SH_PAD / 2);
 }
 template <int N>
 __device__ __forceinline__ void rys_roots(const double* __restrict__ tab, double T, double* __restrict__ x, double* __restrict__ w) {

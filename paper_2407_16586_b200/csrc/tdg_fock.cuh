@@ -95,7 +95,7 @@ __device__ __forceinline__ void quartet_fock(const KParams& P, const PairHdr& bh
         double s2 = 1.0, ss = 1.0;
         if (op == 1) { ss = P.omega * rsqrt(P.omega2 + rho); s2 = ss * ss; }
         double xr[NR], wr[NR];
-        rys_eval<NR>(rys, s2 * T, xr, wr);
+        rys_eval<NR, (NR <= 4)>(rys, s2 * T, xr, wr);
         const double wj = op == 0 ? 1.0 : 0.0, wk = op == 0 ? P.cK : P.cLR;
 #pragma unroll
         for (int r = 0; r < NR; ++r) {
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(TDG_NT) tdg_fock_kernel(const __grid_constant_
   const double* rys = P.rys_tab + rys_part_off(NR);
   if (RYS_SH) {
     const double2* src = reinterpret_cast<const double2*>(rys);
-    for (int i = t; i < rys_part_doubles(NR) / 2; i += TDG_NT) s_dyn[i] = __ldg(src + i);
+    for (int i = t; i < rys_part_doubles(NR) / 2; i += TDG_NT) s_dyn[rys_sh_index<NR>(i)] = __ldg(src + i);   // conflict-free staged layout (tdg_common.cuh)
     rys = reinterpret_cast<const double*>(s_dyn);
   }
   __syncthreads();

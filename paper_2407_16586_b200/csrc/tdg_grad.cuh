@@ -19,6 +19,12 @@
 #ifndef TDG_RU_LIM
 #define TDG_RU_LIM 120
 #endif
+#ifndef TDG_STAGE_IJ
+#define TDG_STAGE_IJ 1
+#endif
+#ifndef TDG_STAGE_IJ_MAXAB
+#define TDG_STAGE_IJ_MAXAB 3   // measured on cfg 3 (profiles/r02_variants.md): -1 % on ss and ps bras, +1..10 % on pp, ds, dp bras
+#endif
 #define TDG_MAX_ROLES_F 8
 #define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dd), f shells) use the block-per-quartet kernel (tdg_gradb.cuh)
 // target number of function quartets per role: 27 is the measured optimum (14: +30 %, 54: +15 % time on cfg 3), except
@@ -49,8 +55,13 @@ struct QC {
   static constexpr int UNR = SMALL ? 64 : 1;
   static constexpr bool TWO_STAGE = SMALL && NROLE <= 2;   // measured: faster for 1-2 roles, slower for classes with more roles
   static constexpr bool RYS_SH = NR <= 4;                                  // Rys table of this NR staged in shared memory
-  static constexpr int RYS_SH_DOUBLES = RYS_SH ? rys_part_doubles(NR) : 0;
+  static constexpr int RYS_SH_DOUBLES = RYS_SH ? rys_sh_doubles(NR) : 0;    // staged size (padded layout, tdg_common.cuh)
+  static constexpr int RYS_SRC_DOUBLES = RYS_SH ? rys_part_doubles(NR) : 0;
   static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
+  // (ij) density blocks of the 32 bras of a tile staged in shared memory, already multiplied by M_J (step a7): bra-invariant over
+  // the kets of the work item, so one global gather per block instead of one per quartet
+  static constexpr bool IJ_SH = TDG_STAGE_IJ && SMALL && NAB <= TDG_STAGE_IJ_MAXAB;
+  static constexpr int IJ_SH_DOUBLES = IJ_SH ? TDG_WARP * NAB * 4 : 0;
 };
 
 // 2-D integrals of one direction for one root: I[i][j][k][l], i<=LA+1, j<=LB+1 (i+j<=LA+LB+1), k<=LC+1, l<=LD.
@@ -136,7 +147,7 @@ template <int LA, int LB, int AB0, int ABC> struct Touch { static constexpr unsi
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh, const double* __restrict__ bprim,
                                              const PairHdr& kh, const double* __restrict__ kprim, double deg,
-                                             const double* __restrict__ rys, double (&g)[9]) {
+                                             const double* __restrict__ rys, const double* __restrict__ sIJ, double (&g)[9]) {
   typedef QC<LA, LB, LC, LD> C;
   constexpr int NA = C::NA, NB = C::NB, NC = C::NC, ND = C::ND, NR = C::NR, U = C::UNR, RU = C::RUNR;
   constexpr bool SM = C::SMALL;
@@ -170,14 +181,21 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
 #pragma unroll(U)
     for (int e = 0; e < NC * ND; ++e) {
       const d4 x = ld256(bKL + 4 * e);
+      if constexpr (C::IJ_SH) { vKL[e][0] = x.x; vKL[e][1] = x.y; vKL[e][2] = x.z; vKL[e][3] = x.w; }   // M_J is already in the staged (ij) block
+      else {
 #pragma unroll
-      for (int m = 0; m < 4; ++m) vKL[e][m] = P.MJ[4 * m] * x.x + P.MJ[4 * m + 1] * x.y + P.MJ[4 * m + 2] * x.z + P.MJ[4 * m + 3] * x.w;
+        for (int m = 0; m < 4; ++m) vKL[e][m] = P.MJ[4 * m] * x.x + P.MJ[4 * m + 1] * x.y + P.MJ[4 * m + 2] * x.z + P.MJ[4 * m + 3] * x.w;
+      }
     }
 #pragma unroll(U)
     for (int ab = AB0; ab < AB0 + ABC; ++ab) {
       {
         const int a = ab / NB, b = ab - a * NB;
-        const d4 jv = ld256(bIJ + 4 * (a * NB + b));
+        d4 jv;
+        if constexpr (C::IJ_SH) {
+          const double2 j0 = *reinterpret_cast<const double2*>(sIJ + 4 * ab), j1 = *reinterpret_cast<const double2*>(sIJ + 4 * ab + 2);
+          jv.x = j0.x; jv.y = j0.y; jv.z = j1.x; jv.w = j1.y;
+        } else jv = ld256(bIJ + 4 * (a * NB + b));
 #pragma unroll(U)
         for (int c = 0; c < NC; ++c) {
           const d4 u = ld256(bIK + 4 * (a * NC + c));
@@ -218,7 +236,7 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
         double s2 = 1.0, ss = 1.0;
         if (op == 1) { ss = P.omega * rsqrt(P.omega2 + rho); s2 = ss * ss; }
         double xr[NR], wr[NR];
-        rys_eval<NR>(rys, s2 * T, xr, wr);
+        rys_eval<NR, C::RYS_SH>(rys, s2 * T, xr, wr);
         const double* __restrict__ G = op == 0 ? GF : GL;
 #pragma unroll(RU)
         for (int r = 0; r < NR; ++r) {
@@ -389,7 +407,8 @@ __device__ __forceinline__ void warp_survivor(unsigned mask, int pre, int s, int
 // Phase 2 of the kernel for one role (slice [AB0, AB0+ABC) of the bra function pairs).
 template <int LA, int LB, int LC, int LD, int AB0, int ABC>
 __device__ __forceinline__ void process_survivors(const KParams& P, const PairHdr* s_bra, const PairHdr* s_ket, unsigned mask, int pre, int tot,
-                                                  double* s_gb, double* s_gk, int bra0, int k0, const double* __restrict__ rys) {
+                                                  double* s_gb, double* s_gk, int bra0, int k0, const double* __restrict__ rys,
+                                                  const double* __restrict__ s_ij) {
   // Each warp owns the 32 kets [32 w, 32 w + 32) of the chunk and takes passes of 32 consecutive entries of its ket-major
   // survivor list.  Gradient accumulation uses no atomics (shared-memory FP64 atomics are CAS loops of ~60 iterations
   // per warp and 6 RED per quartet saturate L2; both measured): lanes with the same ket are contiguous, so the ket-centre
@@ -414,7 +433,8 @@ __device__ __forceinline__ void process_survivors(const KParams& P, const PairHd
       if (kh.ish == kh.jsh) deg *= 0.5;
       if (P.same_bucket && k0 + kw0 + kt == bra0 + b) deg *= 0.5;
       quartet_grad<LA, LB, LC, LD, AB0, ABC>(P, bh, P.bra_prim + (size_t)(bra0 + b) * P.nppb * TDG_PRIM_STRIDE, kh,
-                                             P.ket_prim + (size_t)(k0 + kw0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys, g);
+                                             P.ket_prim + (size_t)(k0 + kw0 + kt) * P.nppk * TDG_PRIM_STRIDE, deg, rys,
+                                             s_ij + b * (QC<LA, LB, LC, LD>::NAB * 4), g);
     } else {
 #pragma unroll
       for (int x = 0; x < 9; ++x) g[x] = 0.0;
@@ -469,7 +489,8 @@ __global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid
   typedef QC<LA, LB, LC, LD> C;
   double* s_gb = reinterpret_cast<double*>(s_dyn);            // [warp][bra][centre A,B][xyz]
   double* s_gk = s_gb + TDG_WARPS * TDG_WARP * 6;             // [ket][centre C,D][xyz]; ket 32 w + o belongs to warp w
-  double2* s_rys = s_dyn + TDG_ACC_DOUBLES / 2;
+  double* s_ij = s_gb + TDG_ACC_DOUBLES;                      // [bra][ab][4]: M_J . pk(ij)  (QC::IJ_SH)
+  double2* s_rys = s_dyn + (TDG_ACC_DOUBLES + C::IJ_SH_DOUBLES) / 2;
   int tile, chunk;
   find_work_item(P, blockIdx.x, tile, chunk);
   const int t = threadIdx.x, lane = t & 31;
@@ -485,10 +506,20 @@ __global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid
   const bool ket_ok = k < P.nket;
   if (ket_ok) s_ket[t] = P.ket_hdr[k];
   for (int i = t; i < TDG_ACC_DOUBLES; i += TDG_NT) s_gb[i] = 0.0;
+  if constexpr (C::IJ_SH) {   // stage M_J . pk(ij)[a,b] of the tile's bras (offsets straight from the global headers: no extra barrier)
+    for (int e = t; e < nb * C::NAB; e += TDG_NT) {
+      const int b = e / C::NAB, ab = e - b * C::NAB;
+      const PairHdr* gh = P.bra_hdr + bra0 + b;
+      const d4 x = ld256(P.pk + 4 * ((size_t)gh->offA * P.nbf + (size_t)C::NA * gh->offB) + 4 * ab);
+      double* dst = s_ij + 4 * e;
+#pragma unroll
+      for (int m = 0; m < 4; ++m) dst[m] = P.MJ[4 * m] * x.x + P.MJ[4 * m + 1] * x.y + P.MJ[4 * m + 2] * x.z + P.MJ[4 * m + 3] * x.w;
+    }
+  }
   const double* rys = P.rys_tab + rys_part_off(C::NR);
   if (C::RYS_SH) {
     const double2* src = reinterpret_cast<const double2*>(rys);
-    for (int i = t; i < C::RYS_SH_DOUBLES / 2; i += TDG_NT) s_rys[i] = __ldg(src + i);
+    for (int i = t; i < C::RYS_SRC_DOUBLES / 2; i += TDG_NT) s_rys[rys_sh_index<C::NR>(i)] = __ldg(src + i);
     rys = reinterpret_cast<const double*>(s_rys);
   }
   __syncthreads();
@@ -504,7 +535,7 @@ __global__ void __launch_bounds__(TDG_NT, TDG_MINB) tdg_grad_kernel(const __grid
   static_assert(ROLE >= 0 && ROLE < C::NROLE, "role out of range");
   constexpr int AB0 = ROLE * C::ABN;
   constexpr int ABC = (AB0 + C::ABN <= C::NAB) ? C::ABN : C::NAB - AB0;
-  process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, mask, incl - cnt, tot, s_gb, s_gk, bra0, k0, rys);
+  process_survivors<LA, LB, LC, LD, AB0, ABC>(P, s_bra, s_ket, mask, incl - cnt, tot, s_gb, s_gk, bra0, k0, rys, s_ij);
   __syncthreads();
   // flush: sum the warps' private bra slots, one FP64 RED per touched (pair, centre, xyz)
   for (int i = t; i < (TDG_WARP + TDG_KB) * 6; i += TDG_NT) {
