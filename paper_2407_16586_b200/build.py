@@ -20,7 +20,8 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 # per-class compile flags: minimum resident blocks per SM of __launch_bounds__ (registers traded for occupancy), measured on
 # cfg 3 (profiles/r02_variants.md): class -> extra nvcc flags
-CLASS_FLAGS: dict = {(0, 0, 0, 0): ["-DTDG_MINB=4"], (1, 0, 0, 0): ["-DTDG_MINB=3"], (2, 0, 0, 0): ["-DTDG_MINB=3"]}
+CLASS_FLAGS: dict = {(0, 0, 0, 0): ["-DTDG_MINB=4", "-DTDG_DUAL_RYS=1"], (1, 0, 0, 0): ["-DTDG_MINB=3"], (2, 0, 0, 0): ["-DTDG_MINB=3"],
+                     (1, 0, 1, 0): ["-DTDG_DUAL_RYS=1"]}   # TDG_DUAL_RYS: both operators' Rys rules evaluated back to back (tdg_grad.cuh)
 
 
 def ncart(l: int) -> int:

@@ -22,6 +22,9 @@
 #ifndef TDG_STAGE_IJ
 #define TDG_STAGE_IJ 1
 #endif
+#ifndef TDG_DUAL_RYS
+#define TDG_DUAL_RYS 0   // per class (build.py CLASS_FLAGS): -4 % on (ps|ps), -1 % on (ss|ss), +5 % on (ds|ss) (spills), neutral on (ps|ss), (pp|ss)
+#endif
 #ifndef TDG_STAGE_IJ_MAXAB
 #define TDG_STAGE_IJ_MAXAB 3   // measured on cfg 3 (profiles/r02_variants.md): -1 % on ss and ps bras, +1..10 % on pp, ds, dp bras
 #endif
@@ -60,6 +63,7 @@ struct QC {
   static constexpr int RUNR = (SMALL && ABN * KDN * NR <= TDG_RU_LIM) ? 64 : 1;   // root loop
   // (ij) density blocks of the 32 bras of a tile staged in shared memory, already multiplied by M_J (step a7): bra-invariant over
   // the kets of the work item, so one global gather per block instead of one per quartet
+  static constexpr bool DUAL_RYS = TDG_DUAL_RYS && NR <= 2;
   static constexpr bool IJ_SH = TDG_STAGE_IJ && SMALL && NAB <= TDG_STAGE_IJ_MAXAB;
   static constexpr int IJ_SH_DOUBLES = IJ_SH ? TDG_WARP * NAB * 4 : 0;
 };
@@ -232,11 +236,26 @@ __device__ __forceinline__ void quartet_grad(const KParams& P, const PairHdr& bh
       const double rs = rsqrt(p + q), rpq = rs * rs, rho = p * q * rpq;
       const double T = rho * (PQx * PQx + PQy * PQy + PQz * PQz);
       const double pref = Kab * kp1.x * rs;
+      // n <= 2: the rules of both operators are evaluated back to back, unconditionally, before the operator loop, so that their
+      // two dependency chains (exp, Taylor row, closed-form roots) interleave; the loop then picks its set with selects
+      double xa[C::DUAL_RYS ? 2 * NR : 1], wa[C::DUAL_RYS ? 2 * NR : 1];
+      if constexpr (C::DUAL_RYS) {
+        const double ssl = P.omega * rsqrt(P.omega2 + rho), s2l = ssl * ssl;   // omega = 0 (no long-range pass): T = 0, unused
+        rys_eval<NR, C::RYS_SH>(rys, T, xa, wa);
+        rys_eval<NR, C::RYS_SH>(rys, s2l * T, xa + NR, wa + NR);
+#pragma unroll
+        for (int r = 0; r < NR; ++r) { xa[NR + r] *= s2l; wa[NR + r] *= ssl; }
+      }
       for (int op = 0; op <= P.use_lr; ++op) {
         double s2 = 1.0, ss = 1.0;
-        if (op == 1) { ss = P.omega * rsqrt(P.omega2 + rho); s2 = ss * ss; }
         double xr[NR], wr[NR];
-        rys_eval<NR, C::RYS_SH>(rys, s2 * T, xr, wr);
+        if constexpr (C::DUAL_RYS) {
+#pragma unroll
+          for (int r = 0; r < NR; ++r) { xr[r] = op == 0 ? xa[r] : xa[NR + r]; wr[r] = op == 0 ? wa[r] : wa[NR + r]; }
+        } else {
+          if (op == 1) { ss = P.omega * rsqrt(P.omega2 + rho); s2 = ss * ss; }
+          rys_eval<NR, C::RYS_SH>(rys, s2 * T, xr, wr);
+        }
         const double* __restrict__ G = op == 0 ? GF : GL;
 #pragma unroll(RU)
         for (int r = 0; r < NR; ++r) {
