@@ -342,7 +342,7 @@ def run_ours(args, backend=None, emit=print):
     # end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region; rank 0 alone for replicas,
     # every rank (partial gradients all-reduced, max over ranks) when the work is sharded
     e2e_dt = None
-    if rank == 0 or shard:
+    if (rank == 0 or shard) and not getattr(args, "no_e2e", False):
         hD, hP, hT = be.host_copies((D, P, T))
         hpairs, _, _ = wl.default_call(hD, hP, hT)
         e2e_warm = 0 if ms / args.steps > 20000 else 1
@@ -363,9 +363,11 @@ def run_ours(args, backend=None, emit=print):
         roofline = roofline_of(agg_ms, agg_q, agg_p, ms if not shard else ms / args.steps, peak_tf, cfg, roof_steps)
         dt = e2e_dt
         h2d = 3 * nbf * nbf * 8 + sysm.xyz.nbytes + sysm.exps.nbytes + sysm.coefs.nbytes + sysm.shells.nbytes
-        e2e = dict(value=((total_quartets if shard else quartets) / args.steps) / dt, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(natom * 3 * 8), seconds=dt)
+        e2e = None if dt is None else dict(value=((total_quartets if shard else quartets) / args.steps) / dt, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(natom * 3 * 8), seconds=dt)
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
+            if e2e_dt is None:
+                hD, hP, hT = be.host_copies((D, P, T))
             cpu = oracle_sample(cfg, sysm, (hD, hP, hT))
             cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "seconds_screening", "seconds_integrals")}
             cpu["note"] = "unoptimised checker (plain C, gcc -O2), not a tuned CPU implementation: the ratio to it is not a speedup claim"
@@ -398,6 +400,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs under ncu; `e2e` is then null)")
     ap.add_argument("--densities", default="dense", choices=["dense", "decaying"],
                     help="dense: BASELINE.json's random matrices; decaying: second workload with spatially decaying densities (NEXT-4)")
     ap.add_argument("--streams", type=int, default=1, help="CUDA streams the class launches of a call are dealt over (tdg_set_streams)")

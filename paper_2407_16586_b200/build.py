@@ -24,6 +24,9 @@ CLASS_FLAGS: dict = {(0, 0, 0, 0): ["-DTDG_MINB=4", "-DTDG_DUAL_RYS=1"], (1, 0, 
                      (1, 0, 1, 0): ["-DTDG_DUAL_RYS=1"]}   # TDG_DUAL_RYS: both operators' Rys rules evaluated back to back (tdg_grad.cuh)
 
 
+MAX_ROLES_F = 15   # TDG_MAX_ROLES_F of csrc/tdg_grad.cuh
+
+
 def ncart(l: int) -> int:
     return (l + 1) * (l + 2) // 2
 
@@ -34,7 +37,7 @@ def num_roles(la: int, lb: int, lc: int, ld: int) -> int:
     nab, kdn = ncart(la) * ncart(lb), ncart(lc) * ncart(ld)
     abn1 = nab if rc // kdn >= nab else max(rc // kdn, 1)
     nrole1 = -(-nab // abn1)
-    small = nab * kdn <= 27 or nrole1 <= (8 if 3 in (la, lb, lc, ld) else 18)
+    small = nab * kdn <= 27 or nrole1 <= (MAX_ROLES_F if 3 in (la, lb, lc, ld) else 18)
     return nrole1 if small else 1
 DEPS = {   # headers each source includes
     "tdg_class.cu": ["tdg_common.cuh", "tdg_grad.cuh", "tdg_gradb.cuh", "tdg_fock.cuh", "rys_meta.inc"],

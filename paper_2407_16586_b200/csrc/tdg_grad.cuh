@@ -28,11 +28,13 @@
 #ifndef TDG_STAGE_IJ_MAXAB
 #define TDG_STAGE_IJ_MAXAB 3   // measured on cfg 3 (profiles/r02_variants.md): -1 % on ss and ps bras, +1..10 % on pp, ds, dp bras
 #endif
-#define TDG_MAX_ROLES_F 8
+#define TDG_MAX_ROLES_F 15   // f classes up to 15 roles run unrolled (cfg 2: 13.1 s -> 9.6 s against 8; each role is a 25-45 s compile)
 #define TDG_MAX_ROLES 18  // classes needing more roles ((dd|dd), f shells) use the block-per-quartet kernel (tdg_gradb.cuh)
 // target number of function quartets per role: 27 is the measured optimum (14: +30 %, 54: +15 % time on cfg 3), except
 // (dd|dp), which needs 54 to stay within TDG_MAX_ROLES (12 roles; 10x faster than the block-per-quartet kernel on cfg 3)
-__host__ __device__ constexpr int role_comps(int la, int lb, int lc, int ld) { return (la == 2 && lb == 2 && lc == 2 && ld == 1) ? 54 : 27; }
+__host__ __device__ constexpr int role_comps(int la, int lb, int lc, int ld) {
+  return (la == 2 && lb == 2 && lc == 2 && ld == 1) ? 54 : 27;
+}
 
 template <int LA, int LB, int LC, int LD>
 struct QC {
@@ -50,7 +52,7 @@ struct QC {
   static constexpr int RC = role_comps(LA, LB, LC, LD);
   static constexpr int ABN1 = RC / KDN >= NAB ? NAB : (RC / KDN > 0 ? RC / KDN : 1);
   static constexpr int NROLE1 = (NAB + ABN1 - 1) / ABN1;
-  // thread-per-quartet, fully unrolled code: up to 18 roles without f shells, up to 8 with (longer compiles; measured on cfg 2:
+  // thread-per-quartet, fully unrolled code: up to 18 roles without f shells, up to 15 with (longer compiles; measured on cfg 2:
   // the block-per-quartet kernel is 5-10x slower on the small f classes, which carry most of that config's quartets)
   static constexpr bool SMALL = NCOMP <= 27 || NROLE1 <= (HASF ? TDG_MAX_ROLES_F : TDG_MAX_ROLES);
   static constexpr int NROLE = SMALL ? NROLE1 : 1;

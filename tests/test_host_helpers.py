@@ -73,4 +73,5 @@ def test_build_role_count_matches_header_formula():
     assert build.num_roles(2, 1, 1, 0) == 2 and build.num_roles(2, 1, 2, 1) == 18 and build.num_roles(2, 2, 2, 1) == 12
     assert build.num_roles(2, 2, 2, 2) == 1 and build.num_roles(3, 0, 0, 0) == 1 and build.num_roles(3, 3, 3, 3) == 1
     assert build.num_roles(3, 1, 1, 0) == 4 and build.num_roles(3, 0, 1, 0) == 2 and build.num_roles(3, 2, 1, 0) == 7
-    assert build.num_roles(3, 1, 1, 1) == 1      # 10 roles: too many for an f class, block-per-quartet kernel
+    assert build.num_roles(3, 1, 1, 1) == 10 and build.num_roles(3, 1, 3, 0) == 15      # f classes: unrolled up to 15 roles
+    assert build.num_roles(3, 2, 1, 1) == 1      # 20 roles: too many for an f class, block-per-quartet kernel
