@@ -26,6 +26,22 @@ def ctx():
     c.close()
 
 
+@pytest.fixture(scope="module")
+def cfg1_case(orc):
+    """cfg 1 inputs and the oracle's full gradient, computed once for the tests that compare against it (24 s of oracle time each)."""
+    s = wl.make_system(1)
+    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
+    pairs, wJ, wK = wl.default_call(D, P, T)
+    ref, rst = orc.gradient(s, pairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"], tau=s.tau, density_weighted=s.density_weighted)
+    return s, pairs, wJ, wK, ref, rst
+
+
+def _run_gpu(ctx, s, pairs, wJ, wK, call=CALL):
+    ctx.set_system(s)
+    ctx.plan(s.tau, s.density_weighted)
+    return ctx.gradient(pairs, wJ, wK, call["cJ"], call["cK"], call["cLR"], call["omega"])
+
+
 def _compare(g, ref):
     d = np.max(np.abs(g - ref))
     assert d <= ABS_TOL, d
@@ -142,11 +158,9 @@ def test_cfg0_golden_and_oracle(ctx, orc):
     assert np.max(np.abs(g.sum(axis=0))) < 1e-10
 
 
-def test_cfg1_full(ctx, orc):
-    s = wl.make_system(1)
-    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
-    pairs, wJ, wK = wl.default_call(D, P, T)
-    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK)
+def test_cfg1_full(ctx, cfg1_case):
+    s, pairs, wJ, wK, ref, rst = cfg1_case
+    g, st = _run_gpu(ctx, s, pairs, wJ, wK)
     _compare(g, ref)
     for k in ("pairs_total", "pairs_kept", "quartets_visited", "quartets_computed", "prim_quartets"):
         assert st[k] == rst[k], (k, st[k], rst[k])
@@ -235,15 +249,13 @@ def test_gpu_gradient_is_derivative_of_gpu_energy(ctx):
 
 
 @pytest.mark.parametrize("nranks", [2, 3])
-def test_sharded_work_items_partition_the_gradient(ctx, orc, nranks):
+def test_sharded_work_items_partition_the_gradient(ctx, cfg1_case, nranks):
     """SURVEY.md 8(e) / PAPER.md:309: the rank shards (tdg_set_shard) partition the quartets exactly (integer counts add up
     to the unsharded ones, class by class) and their partial gradients sum to the oracle's gradient.  The shards run one
     after another on this GPU, each to completion; no rank waits on another."""
-    s = wl.make_system(1)
-    D, P, T = wl.make_densities(s.nbf, wl.density_seed(1))
-    pairs, wJ, wK = wl.default_call(D, P, T)
+    s, pairs, wJ, wK, ref, _ = cfg1_case
     try:
-        g_full, st_full, ref, _ = _run_both(ctx, orc, s, pairs, wJ, wK)
+        g_full, st_full = _run_gpu(ctx, s, pairs, wJ, wK)
         total = np.zeros_like(g_full)
         counts = {k: 0 for k in ("quartets_visited", "quartets_computed", "prim_quartets")}
         by_class = np.zeros(len(st_full["quartets_by_class"]), dtype=np.int64)
@@ -279,10 +291,24 @@ def test_set_shard_rejects_bad_arguments(ctx):
 def test_cfg4_subsample_largest_configuration(ctx, orc):
     """1024 waters (25 600 bf, 21 GB packed densities): deterministic subsample both sides evaluate (S12).
     Last in the file: ~12 min, almost all of it the oracle's own Schwarz bounds over 7.5e7 shell pairs."""
+    import torch
+
     s = wl.make_system(4)
-    D, P, T = wl.make_densities(s.nbf, wl.density_seed(4))
-    pairs, wJ, wK = wl.default_call(D, P, T)
-    g, st, ref, rst = _run_both(ctx, orc, s, pairs, wJ, wK, sample_mod=4000000, sample_seed=4)
+    # densities generated on the device, as bench.py does for cfg 3-4 (the numpy recipe costs minutes of host GEMMs at 25 600 functions);
+    # the CUDA path gets the device tensors, the oracle their host copies: both sides see identical arrays
+    dev = wl.make_densities_torch(s.nbf, 20240716 + 4, "cuda")
+    dpairs, wJ, wK = wl.default_call(*dev)
+    hpairs, _, _ = wl.default_call(*[x.cpu().numpy() for x in dev])
+    tau, dw, mod, seed = s.tau, s.density_weighted, 4000000, 4
+    ctx.set_system(s)
+    ctx.plan(tau, dw, mod, seed)
+    out = torch.zeros((s.natom, 3), dtype=torch.float64, device="cuda")
+    _, st = ctx.gradient(dpairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"], out=out)
+    g = out.cpu().numpy()
+    del dev, dpairs, out
+    torch.cuda.empty_cache()
+    ref, rst = orc.gradient(s, hpairs, wJ, wK, CALL["cJ"], CALL["cK"], CALL["cLR"], CALL["omega"], tau=tau, density_weighted=dw,
+                            sample_mod=mod, sample_seed=seed)
     d = float(np.max(np.abs(g - ref)))
     print("cfg4 subsample: quartets gpu/oracle", st["quartets_computed"], rst["quartets_computed"], "pairs_kept", st["pairs_kept"], rst["pairs_kept"],
           "max|dg|", d, "max|g|", float(np.max(np.abs(ref))))
