@@ -75,3 +75,41 @@ def test_build_role_count_matches_header_formula():
     assert build.num_roles(3, 1, 1, 0) == 4 and build.num_roles(3, 0, 1, 0) == 2 and build.num_roles(3, 2, 1, 0) == 7
     assert build.num_roles(3, 1, 1, 1) == 10 and build.num_roles(3, 1, 3, 0) == 15      # f classes: unrolled up to 15 roles
     assert build.num_roles(3, 2, 1, 1) == 1      # 20 roles: too many for an f class, block-per-quartet kernel
+
+
+def test_bench_roofline_uses_the_capture_only_when_it_matches_the_build(monkeypatch):
+    """bench.roofline_of: executed FLOPs come from the hash-stamped ncu capture under profiles/; a capture taken on other kernel
+    sources, or on another workload (different per-class quartet count), gives null instead of a stale number."""
+    import json
+    import os
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    import bench
+    from paper_2407_16586_b200 import ncu_classes, tdgrad
+
+    cap = json.load(open(os.path.join(root, "profiles", "r02_ncu_classes_cfg3.json")))
+    name = "(ps|ss)"
+    top = [c for c in range(tdgrad.NCLASS) if tdgrad.class_name(c) == name][0]
+    steps = 2
+    ms, q, p = [0.0] * tdgrad.NCLASS, [0] * tdgrad.NCLASS, [0] * tdgrad.NCLASS
+    ms[top] = 1300.0 * steps
+    q[top] = cap["quartets_by_class"][name] * steps
+    p[top] = cap["prim_quartets_by_class"][name] * steps
+    monkeypatch.setattr(ncu_classes, "source_hash", lambda: cap["source_hash"])
+    r = bench.roofline_of(ms, q, p, 9000.0 * steps, 34.2, 3, steps)
+    assert r["kernel"].endswith(name) and r["capture_hash"] == cap["source_hash"]
+    want = cap["classes"][name]["flops"] / 1.3 * 1e-12                      # executed FLOPs of one call / 1.3 s
+    assert abs(r["achieved"] - want) < 1e-9 * want and abs(r["frac"] - want / 34.2) < 1e-12
+    assert r["traffic"] == cap["classes"][name]["dram_read"] + cap["classes"][name]["dram_write"]
+    assert 0.0 < r["frac"] < 1.0 and r["model_frac"] is not None
+    # other kernel sources
+    monkeypatch.setattr(ncu_classes, "source_hash", lambda: "0123456789abcdef")
+    r2 = bench.roofline_of(ms, q, p, 9000.0 * steps, 34.2, 3, steps)
+    assert r2["achieved"] is None and r2["frac"] is None and "older than the kernel sources" in r2["note"]
+    # same sources, other workload
+    monkeypatch.setattr(ncu_classes, "source_hash", lambda: cap["source_hash"])
+    q[top] += 1
+    r3 = bench.roofline_of(ms, q, p, 9000.0 * steps, 34.2, 3, steps)
+    assert r3["frac"] is None and "different workload" in r3["note"]
