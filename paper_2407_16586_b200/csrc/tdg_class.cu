@@ -20,7 +20,7 @@ static void launch(const KParams& P, int nblocks, cudaStream_t s) {
     typedef QB<TDG_LA, TDG_LB, TDG_LC, TDG_LD> B;
     constexpr int smem = B::SMEM_DOUBLES * (int)sizeof(double);
     cudaFuncSetAttribute(tdg_gradb_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    tdg_gradb_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, 0><<<nblocks, B::G, smem, s>>>(P);
+    tdg_gradb_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, 0><<<dim3(nblocks, TDG_GRADB_SLICES), B::G, smem, s>>>(P);
   }
 }
 // Fock-type build of the same (class, role) (NEXT-1; tdg_fock.cuh / MODE 1 of tdg_gradb.cuh)
@@ -35,7 +35,7 @@ static void launch_fock(const KParams& P, int nblocks, cudaStream_t s) {
     typedef QB<TDG_LA, TDG_LB, TDG_LC, TDG_LD> B;
     constexpr int smem = B::SMEM_DOUBLES * (int)sizeof(double);
     cudaFuncSetAttribute(tdg_gradb_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    tdg_gradb_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, 1><<<nblocks, B::G, smem, s>>>(P);
+    tdg_gradb_kernel<TDG_LA, TDG_LB, TDG_LC, TDG_LD, 1><<<dim3(nblocks, TDG_GRADB_SLICES), B::G, smem, s>>>(P);
   }
 }
 namespace {

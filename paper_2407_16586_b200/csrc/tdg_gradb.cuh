@@ -17,6 +17,7 @@
 // Work items, screening (phase 1) and counters are those of tdg_grad.cuh, so the planner does not distinguish the two.
 #pragma once
 #include "tdg_grad.cuh"
+#define TDG_GRADB_SLICES 16   // grid.y of the block-per-quartet kernel: slices of a work item's 128 kets
 
 template <int LA, int LB, int LC, int LD>
 struct QB {
@@ -75,7 +76,10 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
   __syncthreads();
   // ---- phase 1 (step a4): the block's threads share the 128 kets of the chunk ----
   unsigned long long n_vis = 0, n_cmp = 0;
-  for (int kt = t; kt < TDG_KB; kt += G) {
+  // The classes of this kernel have few shell pairs, hence few work items (cfg 3 (dd|dd): 36): a work item is therefore cut into
+  // gridDim.y slices, slice y taking the kets y, y + gridDim.y, ... of the chunk (screening and counters included), so that the launch
+  // fills the GPU (ncu round 2: 4 warps per SM active with one block per work item).
+  for (int kt = blockIdx.y + gridDim.y * t; kt < TDG_KB; kt += gridDim.y * G) {
     const int k = k0 + kt;
     s_mask[kt] = k < P.nket ? screen_ket(P, P.bra_hdr + bra0, s_dij, nb, bra0, k, P.ket_hdr[k], dw, n_vis, n_cmp) : 0u;
   }
@@ -84,7 +88,7 @@ __global__ void __launch_bounds__(QB<LA, LB, LC, LD>::G) tdg_gradb_kernel(const 
   const size_t n = (size_t)P.nbf;
   const double* __restrict__ pk = P.pk;
   // ---- phase 2: survivors one after another, the whole block on each ----
-  for (int kt = 0; kt < TDG_KB; ++kt) {
+  for (int kt = blockIdx.y; kt < TDG_KB; kt += gridDim.y) {
     unsigned m = s_mask[kt];
     if (!m) continue;
     const PairHdr kh = P.ket_hdr[k0 + kt];
